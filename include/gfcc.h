@@ -1,0 +1,124 @@
+/* =====================================================================================
+ * gfcc.h -- C ABI of the B200-native GFCCSD-IP hot path (libgfcc_b200.so).
+ *
+ * The library computes, entirely in hand-written CUDA kernels for sm_100a:
+ *   gfcc_create    one-time similarity-transformed-Hamiltonian intermediates
+ *                  ("constant intermediate tensors ... pre-computed")
+ *   gfcc_sigma_ip  the batched complex matvec  sigma = (omega + Hbar_N - i eta) X  on IP-type
+ *                  vectors X_p(omega) = (X1_i, X2_ija)            (Eq. 3, Eq. 5;
+ *                  "GFCC singles / doubles equations", Alg. 1)
+ *   gfcc_solve_ip  batched GMRES for Eq. 5 (Alg. 1) and the assembly
+ *                  G_pq(omega) = <Phi|(1+Lambda1+Lambda2) abar_q^+ (X_p1 + X_p2)|Phi>
+ *                  (first, IP term of Eq. 7-8)
+ * The working equations (the paper prints none) are SURVEY.md section 8(c); readings are in DESIGN.md.
+ *
+ * Conventions
+ *   spin-orbitals, N = o + v, occupied first.  i,j,m,n occupied in [0,o); a,b,e,f virtual in [0,v).
+ *   <pq|rs> = sum_Q L[Q,p,r] L[Q,q,s];  all of fock, T1, T2, Lambda1, Lambda2, L are REAL FP64.
+ *   complex = interleaved (re, im) pairs of FP64 (layout of cuDoubleComplex / std::complex<double>).
+ *   pair(i<j)  = i*o - i*(i+1)/2 + (j-i-1)          (npair = o(o-1)/2)
+ *   tri(a<b)   = a*v - a*(a+1)/2 + (b-a-1)          (ntri  = v(v-1)/2)
+ *
+ * Pointers: every array argument is a DEVICE pointer unless marked [host].  The *_host entry points
+ * take HOST pointers for the vectors and do the host<->device copies themselves.
+ * Ownership: inputs are read-only.  gfcc_create copies or derives everything it needs EXCEPT T2 and
+ * L2, which are BORROWED: they must stay valid and unmodified until gfcc_destroy (T2 is 56 GB and
+ * Lambda2 28 GB at config 4; they are not duplicated).  fock, T1, L1, Lchol may be freed when
+ * gfcc_create returns.  Outputs are caller-allocated and fully overwritten.
+ * Errors: every call returns 0 on success or a negative GFCC_E* code; no exception or abort crosses
+ * the boundary.  gfcc_last_error(h) gives a message for the last failing call on that handle
+ * (gfcc_last_error(NULL): last failure of gfcc_create on this thread).
+ * Streams: work is enqueued on the handle's stream (default: the legacy default stream; see
+ * gfcc_set_stream).  gfcc_create and gfcc_solve_ip synchronise that stream before returning;
+ * gfcc_sigma_ip is asynchronous with respect to the host.
+ * There is no CPU fallback: without a CUDA device every call fails with GFCC_ECUDA.
+ * ===================================================================================== */
+#ifndef GFCC_H_
+#define GFCC_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GFCC_OK       0
+#define GFCC_EINVAL  -1   /* null pointer, non-positive size, index out of range, unknown option */
+#define GFCC_ENOMEM  -2   /* device allocation failed */
+#define GFCC_ECUDA   -3   /* CUDA runtime error (message in gfcc_last_error) */
+#define GFCC_ENOCONV -4   /* GMRES hit max iterations for at least one right-hand side; G is still written */
+
+typedef struct gfcc_ctx* gfcc_handle;
+
+/* Build the one-time intermediates on the device:
+ *   T1-dressed Cholesky blocks, dressed Fock, F_mi, F_ae, F_me, M^Q_ia, W_mnij (o^4, pair-packed),
+ *   W_mbij (o^3 v, pair-packed), D_ki for the G assembly.
+ * fock  [N][N] row-major (general: f_ov may be non-zero)
+ * T1,L1 [o][v]
+ * T2    pair-packed [npair][v][v]:  T2[pair(i,j)][a][b] = t[i,j,a,b], i<j  (antisymmetric in a,b)   BORROWED
+ * L2    fully packed [npair][ntri]: L2[pair(i,j)][tri(a,b)] = lambda[i,j,a,b], i<j, a<b               BORROWED
+ * Lchol [Q][N][N]
+ * o >= 2, v >= 2, Q >= 1.                                                                            */
+int gfcc_create(int o, int v, int Q, const double* fock, const double* T1, const double* T2, const double* L1,
+                const double* L2, const double* Lchol, gfcc_handle* out);
+
+/* sigma_r = (omega[r] - i eta) X_r + Hbar X_r for r = 0..nrhs-1.
+ * omega [host][nrhs];  X1,S1 complex [nrhs][o];  X2,S2 complex [nrhs][o][o][v].
+ * Precondition (unchecked): X2[r][i][j][a] = -X2[r][j][i][a].  S2 is returned antisymmetric.        */
+int gfcc_sigma_ip(gfcc_handle h, int nrhs, const double* omega, double eta, const void* X1, const void* X2,
+                  void* S1, void* S2);
+/* same, X1,X2,S1,S2 are HOST pointers (pinned or pageable); copies are part of the call; synchronous. */
+int gfcc_sigma_ip_host(gfcc_handle h, int nrhs, const double* omega, double eta, const void* X1, const void* X2,
+                       void* S1, void* S2);
+
+/* Solve (omega_w + Hbar - i eta) X = b_p for every (p[ip], omega[iw]) with batched GMRES
+ * (classical Gram-Schmidt with re-orthogonalisation, complex Givens least squares; restart length,
+ * max iterations and initial guess are options) and assemble
+ *   G[iw][ip][iq] = G_{p[ip], q = p[iq]}(omega[iw])       complex [nw][np][np]
+ * p [host][np] spin-orbital indices in [0,N) (occupied or virtual);  omega [host][nw].
+ * Right-hand sides are ordered r = ip*nw + iw.  G may be a device or a host pointer.
+ * Stop test: |rotated residual| <= tol * ||b||.  Returns GFCC_ENOCONV if some RHS did not converge
+ * (statistics tell which).  X1out/X2out of gfcc_solve_ip_x (nullable, device, layouts of gfcc_sigma_ip
+ * with nrhs = np*nw) receive the solutions.                                                          */
+int gfcc_solve_ip(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol, void* G);
+int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol,
+                    void* G, void* X1out, void* X2out);
+
+/* stream is a cudaStream_t passed as void* (e.g. torch.cuda.current_stream().cuda_stream). */
+int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
+
+/* Options (double-valued):
+ *   "gmres_m"      restart length (default 50; clipped to what device memory allows)
+ *   "gmres_maxit"  maximum number of sigma applications per solve (default 1000)
+ *   "gmres_fixed"  if > 0: run exactly this many Arnoldi steps in ONE cycle, no stop test (timing mode)
+ *   "x0"           0: zero initial guess, 1: zeroth-order guess b/(omega - i eta + d) (default 1)
+ *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3e9)
+ *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256) */
+int gfcc_set_option(gfcc_handle h, const char* key, double val);
+
+/* Statistics of the last call (double-valued): "iterations" (Arnoldi steps of the last solve),
+ * "sigma_applications", "flops_sigma" (executed FP64 flop model of ONE batched application),
+ * "flops_create", "bytes_device" (device memory owned by the handle), "max_relres", "n_unconverged",
+ * "gemm_launches", "kernel_launches" (since create or the last reset by reading "reset_counters"). */
+int gfcc_get_stat(gfcc_handle h, const char* key, double* val);
+/* per right-hand-side results of the last solve: relres [host][n], iters [host][n], n = np*nw.        */
+int gfcc_get_residuals(gfcc_handle h, int n, double* relres, int* iters);
+
+/* Copy a named intermediate to a caller buffer (device pointer, FP64), for parity tests:
+ *   "Fme" [o][v], "Fmi" [o][o], "Fae" [v][v], "Wmnij" packed [npair(i<j)][npair(m<n)],
+ *   "Wmbij" packed [npair(i<j)][v][o] holding W_mbij[m,a,j,i] at [pair(i,j)][a][m], "D" [o][o],
+ *   "Lm" [Q][o][v].  Returns the element count (>0), or <0 on error; out may be NULL to query size.   */
+long long gfcc_get_intermediate(gfcc_handle h, const char* name, double* out);
+
+const char* gfcc_last_error(gfcc_handle h);
+int gfcc_destroy(gfcc_handle h);
+
+/* The FP64 tensor-core GEMM engine every large contraction goes through (exported for unit tests):
+ *   C[m,n] = alpha * sum_k A[m,k] B[k,n] + beta * C[m,n],  element addresses
+ *   A + m*sAm + k*sAk,  B + k*sBk + n*sBn,  C + m*sCm + n*sCn   (exactly one of sAm/sAk and one of
+ *   sBk/sBn must be 1).  DMMA m8n8k4 (mma.sync f64), cp.async multi-stage shared-memory pipeline.     */
+int gfcc_dgemm(void* cuda_stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
+               const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GFCC_H_ */

@@ -1,0 +1,526 @@
+// =====================================================================================
+// gfcc_kernels.cuh -- bandwidth-bound and small kernels of the GFCCSD-IP path (sm_100a).
+//
+// Internal vector layout ("RHS-fastest"): a batch of nrhs complex vectors is a REAL matrix
+//   vec[n][Nc],  Nc = 2*nrhs (column 2r = Re, 2r+1 = Im of right-hand side r),
+//   rows 0..o-1 = x1[i], rows o + pair(i<j)*v + a = x2[i,j,a]   (n = o + npair*v).
+// Because Hbar is real, every contraction acts on the Nc real columns independently
+// ("complex-real mixed operations"; SURVEY.md 8c point 20).
+// =====================================================================================
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gfcc {
+
+__host__ __device__ inline long long pair_index(int i, int j, int o) {
+  return (long long)i * o - (long long)i * (i + 1) / 2 + (j - i - 1);
+}
+__host__ __device__ inline long long tri_index(int a, int b, int v) {
+  return (long long)a * v - (long long)a * (a + 1) / 2 + (b - a - 1);
+}
+
+// inverse of pair_index: packed index pr -> (i<j)
+__host__ __device__ inline void decode_pair(long long pr, int o, int& i, int& j) {
+  const double t = 2.0 * o - 1.0;
+  int ii = (int)((t - sqrt(t * t - 8.0 * (double)pr)) * 0.5);
+  if (ii < 0) ii = 0;
+  if (ii > o - 2) ii = o - 2;
+  while (ii > 0 && pair_index(ii, ii + 1, o) > pr) --ii;
+  while (ii + 2 < o && pair_index(ii + 1, ii + 2, o) <= pr) ++ii;
+  i = ii;
+  j = (int)(pr - pair_index(ii, ii + 1, o)) + ii + 1;
+}
+
+// ------------------------------------------------------------------------------------
+// dst[q][r][c] = src[q][row0 + r][col0 + c]            (transpose == 0)
+// dst[q][r][c] = src[q][row0 + c][col0 + r]            (transpose == 1)   src is [Q][N][N]
+// 32x32 shared-memory tiles so that both sides are coalesced.
+// ------------------------------------------------------------------------------------
+__global__ void k_copy_block(double* __restrict__ dst, const double* __restrict__ src, int R, int Cc, int row0, int col0,
+                             int N, int transpose) {
+  __shared__ double tile[32][33];
+  const int q = blockIdx.z;
+  const double* s = src + (long long)q * N * N;
+  double* d = dst + (long long)q * R * Cc;
+  const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+  if (!transpose) {
+    for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+      const int r = r0 + rr, c = c0 + threadIdx.x;
+      if (r < R && c < Cc) d[(long long)r * Cc + c] = s[(long long)(row0 + r) * N + col0 + c];
+    }
+  } else {
+    // read src rows (row0 + c) with r fastest: src[row0 + c][col0 + r]
+    for (int cc = threadIdx.y; cc < 32; cc += blockDim.y) {
+      const int c = c0 + cc, r = r0 + threadIdx.x;
+      if (r < R && c < Cc) tile[cc][threadIdx.x] = s[(long long)(row0 + c) * N + col0 + r];
+    }
+    __syncthreads();
+    for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+      const int r = r0 + rr, c = c0 + threadIdx.x;
+      if (r < R && c < Cc) d[(long long)r * Cc + c] = tile[threadIdx.x][rr];
+    }
+  }
+}
+
+// s[q] = sum_{k,c} t1[k,c] Lov[q][k][c]
+__global__ void k_sq(double* __restrict__ s, const double* __restrict__ t1, const double* __restrict__ Lov, int ov) {
+  __shared__ double red[256];
+  const int q = blockIdx.x;
+  double acc = 0;
+  for (int k = threadIdx.x; k < ov; k += blockDim.x) acc += t1[k] * Lov[(long long)q * ov + k];
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s2 = blockDim.x / 2; s2 > 0; s2 >>= 1) {
+    if (threadIdx.x < s2) red[threadIdx.x] += red[threadIdx.x + s2];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) s[q] = red[0];
+}
+
+// g[p][q] = f[p][q] + sum_Q s[Q] L[Q][p][q] - Kmat[p][q]
+__global__ void k_fock_jk(double* __restrict__ g, const double* __restrict__ f, const double* __restrict__ s,
+                          const double* __restrict__ L, const double* __restrict__ Kmat, int N, int Q) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)N * N) return;
+  double acc = f[idx] - Kmat[idx];
+  for (int q = 0; q < Q; ++q) acc += s[q] * L[(long long)q * N * N + idx];
+  g[idx] = acc;
+}
+
+// tmp = A^T g ;  A = 1 - t1 on the [occ, virt] block   -> tmp[p][q] = g[p][q] - (p virtual) sum_m t1[m,a] g[m][q]
+__global__ void k_dress_left(double* __restrict__ tmp, const double* __restrict__ g, const double* __restrict__ t1, int o,
+                             int v) {
+  const int N = o + v;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)N * N) return;
+  const int p = idx / N, q = idx % N;
+  double acc = g[idx];
+  if (p >= o) {
+    const int a = p - o;
+    for (int m = 0; m < o; ++m) acc -= t1[(long long)m * v + a] * g[(long long)m * N + q];
+  }
+  tmp[idx] = acc;
+}
+// ft = tmp B ;  B = 1 + t1^T on the [virt, occ] block   -> ft[p][q] = tmp[p][q] + (q occupied) sum_e t1[q,e] tmp[p][o+e]
+__global__ void k_dress_right(double* __restrict__ ft, const double* __restrict__ tmp, const double* __restrict__ t1, int o,
+                              int v) {
+  const int N = o + v;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)N * N) return;
+  const int p = idx / N, q = idx % N;
+  double acc = tmp[idx];
+  if (q < o)
+    for (int e = 0; e < v; ++e) acc += t1[(long long)q * v + e] * tmp[(long long)p * N + o + e];
+  ft[idx] = acc;
+}
+
+// copy a block of the dressed Fock: dst[r][c] = ft[row0 + r][col0 + c]
+__global__ void k_fock_block(double* __restrict__ dst, const double* __restrict__ ft, int R, int Cc, int row0, int col0,
+                             int N) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)R * Cc) return;
+  const int r = idx / Cc, c = idx % Cc;
+  dst[idx] = ft[(long long)(row0 + r) * N + col0 + c];
+}
+
+// Lm[q][i][a] -= Mq[q][i][a]
+__global__ void k_sub(double* __restrict__ dst, const double* __restrict__ src, long long n) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    dst[i] -= src[i];
+}
+__global__ void k_scale(double* __restrict__ dst, double s, long long n) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    dst[i] *= s;
+}
+
+// ------------------------------------------------------------------------------------
+// split-K reduction: C(m,n) = alpha * sum_s part[s][m][n] + beta * C(m,n) with two-level scatter
+// ------------------------------------------------------------------------------------
+__global__ void k_splitk_reduce(double* __restrict__ C, const double* __restrict__ part, int S, int M, int N, double alpha,
+                                double beta, long long sCm0, long long sCm1, int Md, long long sCn0, long long sCn1, int Nd) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)M * N) return;
+  const int m = idx / N, n = idx % N;
+  double acc = 0;
+  for (int s = 0; s < S; ++s) acc += part[(long long)s * M * N + idx];
+  double* p = C + (long long)(m / Md) * sCm1 + (long long)(m % Md) * sCm0 + (long long)(n / Nd) * sCn1 + (long long)(n % Nd) * sCn0;
+  *p = alpha * acc + (beta != 0.0 ? beta * *p : 0.0);
+}
+
+// ------------------------------------------------------------------------------------
+// P5/P6 scatter kernels (create)
+// ------------------------------------------------------------------------------------
+// G1p[(i',m)][(j,n)] for i = i0 + i' :  mode 0: Wp[(i<j)][(m<n)] += G1 (pairs with i<j);
+//                                        mode 1: Wp[(j<i)][(m<n)] -= G1 (pairs with j<i).
+// Two launches per panel so that no address is touched twice inside one launch (deterministic, race-free).
+__global__ void k_scatter_oooo(double* __restrict__ Wp, const double* __restrict__ G1p, int o, int i0, int ni, int mode) {
+  const long long npair = (long long)o * (o - 1) / 2;
+  const long long total = (long long)ni * o * npair;   // (i', j, (m<n))
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const long long mn = idx % npair;
+    const int j = (idx / npair) % o;
+    const int ip = idx / (npair * o);
+    const int i = i0 + ip;
+    if (i == j || (mode == 0) != (i < j)) continue;
+    int m, n;
+    decode_pair(mn, o, m, n);
+    const double val = G1p[((long long)ip * o + m) * ((long long)o * o) + (long long)j * o + n];
+    if (i < j) Wp[pair_index(i, j, o) * npair + mn] += val;
+    else Wp[pair_index(j, i, o) * npair + mn] -= val;
+  }
+}
+// tmp[(i<j)][(m', n')] (m = m0+m', n = nlo + n', ncols = o - nlo) : Wp[(i<j)][(m<n)] += sign * tmp for m<n
+__global__ void k_pack_oooo_cols(double* __restrict__ Wp, const double* __restrict__ tmp, int o, int m0, int nm, int nlo,
+                                 double sign) {
+  const long long npair = (long long)o * (o - 1) / 2;
+  const int ncols = o - nlo;
+  const long long total = npair * nm * ncols;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int np_ = idx % ncols;
+    const int mp = (idx / ncols) % nm;
+    const long long ij = idx / ((long long)ncols * nm);
+    const int m = m0 + mp, n = nlo + np_;
+    if (m < n) Wp[ij * npair + pair_index(m, n, o)] += sign * tmp[idx];
+  }
+}
+// X1p[(i',m)][(j,b)] (i = i0+i'):  Wacc[(i<j)][b][m] += X (i<j);  Wacc[(j<i)][b][m] -= X (j<i)
+__global__ void k_scatter_ovoo(double* __restrict__ Wacc, const double* __restrict__ Xp, int o, int v, int i0, int ni, int mode) {
+  const long long total = (long long)ni * o * o * v;   // (i', j, b, m)  -- m fastest for coalesced writes
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int m = idx % o;
+    const int b = (idx / o) % v;
+    const int j = (idx / ((long long)o * v)) % o;
+    const int ip = idx / ((long long)o * v * o);
+    const int i = i0 + ip;
+    if (i == j || (mode == 0) != (i < j)) continue;
+    const double val = Xp[((long long)ip * o + m) * ((long long)o * v) + (long long)j * v + b];
+    if (i < j) Wacc[(pair_index(i, j, o) * v + b) * o + m] += val;
+    else Wacc[(pair_index(j, i, o) * v + b) * o + m] -= val;
+  }
+}
+// X2p[j][(i',m)][b] (i = i0+i'): same scatter rule
+__global__ void k_scatter_ovoo_batched(double* __restrict__ Wacc, const double* __restrict__ Xp, int o, int v, int i0, int ni, int mode) {
+  const long long total = (long long)o * ni * o * v;   // (j, i', b, m)
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int m = idx % o;
+    const int b = (idx / o) % v;
+    const int ip = (idx / ((long long)o * v)) % ni;
+    const int j = idx / ((long long)o * v * ni);
+    const int i = i0 + ip;
+    if (i == j || (mode == 0) != (i < j)) continue;
+    const double val = Xp[(((long long)j * ni + ip) * o + m) * v + b];
+    if (i < j) Wacc[(pair_index(i, j, o) * v + b) * o + m] += val;
+    else Wacc[(pair_index(j, i, o) * v + b) * o + m] -= val;
+  }
+}
+
+// gather rows for D: TJ[k][(a,b)] = t[k,j,a,b] (full v*v, from pair-packed T2), LJ[i][(a,b)] = lambda[i,j,a,b] (from [a<b] packed)
+__global__ void k_gather_t2_rows(double* __restrict__ TJ, const double* __restrict__ T2p, int o, int v, int j) {
+  const long long vv = (long long)v * v;
+  const long long total = (long long)o * vv;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int k = idx / vv;
+    const long long ab = idx % vv;
+    double val = 0.0;
+    if (k < j) val = T2p[pair_index(k, j, o) * vv + ab];
+    else if (k > j) val = -T2p[pair_index(j, k, o) * vv + ab];
+    TJ[idx] = val;
+  }
+}
+__global__ void k_gather_l2_rows(double* __restrict__ LJ, const double* __restrict__ L2p, int o, int v, int j) {
+  const long long vv = (long long)v * v, nt = (long long)v * (v - 1) / 2;
+  const long long total = (long long)o * vv;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int i = idx / vv;
+    const int a = (idx % vv) / v, b = idx % v;
+    double val = 0.0;
+    if (i != j && a != b) {
+      double s = 1.0;
+      int ii = i, jj = j, aa = a, bb = b;
+      if (ii > jj) { int t = ii; ii = jj; jj = t; s = -s; }
+      if (aa > bb) { int t = aa; aa = bb; bb = t; s = -s; }
+      val = s * L2p[pair_index(ii, jj, o) * nt + tri_index(aa, bb, v)];
+    }
+    LJ[idx] = val;
+  }
+}
+// D[k][i] = sum_a t1[k,a] l1[i,a]    (initialisation; the doubles part is accumulated by GEMMs)
+__global__ void k_D_singles(double* __restrict__ D, const double* __restrict__ t1, const double* __restrict__ l1, int o, int v) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= o * o) return;
+  const int k = idx / o, i = idx % o;
+  double acc = 0;
+  for (int a = 0; a < v; ++a) acc += t1[(long long)k * v + a] * l1[(long long)i * v + a];
+  D[idx] = acc;
+}
+
+// ------------------------------------------------------------------------------------
+// layout conversion between the C-ABI vectors and the internal RHS-fastest vectors
+// ------------------------------------------------------------------------------------
+// X1 [nrhs][o] complex, X2 [nrhs][o][o][v] complex  ->  vec[n][Nc]  (reads the i<j half of X2)
+__global__ void k_abi_to_vec(double* __restrict__ vec, const double2* __restrict__ X1, const double2* __restrict__ X2, int o,
+                             int v, int nrhs) {
+  // one block per packed row block: blockIdx.x over rows (o singles rows + npair*v doubles rows) in chunks of 32 rows
+  __shared__ double2 tile[32][33];
+  const long long npair = (long long)o * (o - 1) / 2;
+  const long long n = o + npair * v;
+  const long long row0 = (long long)blockIdx.x * 32;
+  const int r0 = blockIdx.y * 32;
+  const int Nc = 2 * nrhs;
+  // load: thread (x = row within 32 [contiguous in a for doubles rows], y = rhs)
+  for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+    const int r = r0 + rr;
+    const long long row = row0 + threadIdx.x;
+    if (r < nrhs && row < n) {
+      double2 val;
+      if (row < o) val = X1[(long long)r * o + row];
+      else {
+        const long long q = row - o;
+        const long long pr = q / v;
+        const int a = q % v;
+        int i, j;
+        decode_pair(pr, o, i, j);
+        val = X2[(((long long)r * o + i) * o + j) * v + a];
+      }
+      tile[rr][threadIdx.x] = val;
+    }
+  }
+  __syncthreads();
+  for (int rw = threadIdx.y; rw < 32; rw += blockDim.y) {
+    const long long row = row0 + rw;
+    const int r = r0 + threadIdx.x;
+    if (r < nrhs && row < n) reinterpret_cast<double2*>(vec + row * Nc)[r] = tile[threadIdx.x][rw];
+  }
+}
+// vec[n][Nc] -> S1 [nrhs][o], S2 [nrhs][o][o][v] complex, antisymmetric fill, zero diagonal
+__global__ void k_vec_to_abi(double2* __restrict__ S1, double2* __restrict__ S2, const double* __restrict__ vec, int o, int v,
+                             int nrhs) {
+  __shared__ double2 tile[32][33];
+  const long long npair = (long long)o * (o - 1) / 2;
+  const long long n = o + npair * v;
+  const long long row0 = (long long)blockIdx.x * 32;
+  const int r0 = blockIdx.y * 32;
+  const int Nc = 2 * nrhs;
+  for (int rw = threadIdx.y; rw < 32; rw += blockDim.y) {
+    const long long row = row0 + rw;
+    const int r = r0 + threadIdx.x;
+    if (r < nrhs && row < n) tile[threadIdx.x][rw] = reinterpret_cast<const double2*>(vec + row * Nc)[r];
+  }
+  __syncthreads();
+  for (int rr = threadIdx.y; rr < 32; rr += blockDim.y) {
+    const int r = r0 + rr;
+    const long long row = row0 + threadIdx.x;
+    if (r < nrhs && row < n) {
+      const double2 val = tile[rr][threadIdx.x];
+      if (row < o) S1[(long long)r * o + row] = val;
+      else {
+        const long long q = row - o;
+        const long long pr = q / v;
+        const int a = q % v;
+        int i, j;
+        decode_pair(pr, o, i, j);
+        S2[(((long long)r * o + i) * o + j) * v + a] = val;
+        S2[(((long long)r * o + j) * o + i) * v + a] = make_double2(-val.x, -val.y);
+      }
+    }
+  }
+}
+__global__ void k_zero_diag(double2* __restrict__ S2, int o, int v, int nrhs) {
+  const long long total = (long long)nrhs * o * v;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int a = idx % v;
+    const int i = (idx / v) % o;
+    const int r = idx / ((long long)v * o);
+    S2[(((long long)r * o + i) * o + i) * v + a] = make_double2(0.0, 0.0);
+  }
+}
+
+// XU[m][e][j][c] = x2[m,j,e,c]   from the packed vector (rows o + pair*v + e), antisymmetric fill
+__global__ void k_unpack_xu(double* __restrict__ XU, const double* __restrict__ vec, int o, int v, int Nc) {
+  // grid: (m*v + e) in blockIdx.x ; threads over (j, c)
+  const int m = blockIdx.x / v, e = blockIdx.x % v;
+  double* dst = XU + (long long)blockIdx.x * o * Nc;
+  const double* x2 = vec + (long long)o * Nc;
+  for (int t = threadIdx.x; t < o * Nc; t += blockDim.x) {
+    const int j = t / Nc, c = t % Nc;
+    double val = 0.0;
+    if (m < j) val = x2[(pair_index(m, j, o) * v + e) * Nc + c];
+    else if (m > j) val = -x2[(pair_index(j, m, o) * v + e) * Nc + c];
+    dst[t] = val;
+  }
+}
+
+// K2P[(i',a)][(m,e)] += delta_ae Fmi[m][i] - 1/2 delta_im Fae[a][e]      (folds sigma2 terms A and B into the ring panel)
+__global__ void k_k2_fixup(double* __restrict__ K2P, const double* __restrict__ Fmi, const double* __restrict__ Fae, int o, int v,
+                           int i0) {
+  const int row = blockIdx.x;   // (i', a)
+  const int ip = row / v, a = row % v;
+  const int i = i0 + ip;
+  double* r = K2P + (long long)row * o * v;
+  for (int t = threadIdx.x; t < o + v; t += blockDim.x) {
+    if (t < o) {
+      const int m = t;
+      double add = Fmi[(long long)m * o + i];
+      if (m == i) add -= 0.5 * Fae[(long long)a * v + a];
+      r[(long long)m * v + a] += add;
+    } else {
+      const int e = t - o;
+      if (e != a) r[(long long)i * v + e] -= 0.5 * Fae[(long long)a * v + e];
+    }
+  }
+}
+
+// sigma1 small terms: s1[i][c] += shift_c * x1[i][c] - sum_m Fmi[m][i] x1[m][c]
+__global__ void k_sigma1_small(double* __restrict__ sout, const double* __restrict__ xin, const double* __restrict__ Fmi,
+                               const double* __restrict__ omega, double eta, int o, int nrhs) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;   // (i, r)
+  if (idx >= o * nrhs) return;
+  const int i = idx / nrhs, r = idx % nrhs;
+  const int Nc = 2 * nrhs;
+  const double2 x = reinterpret_cast<const double2*>(xin + (long long)i * Nc)[r];
+  const double w = omega[r];
+  double re = w * x.x + eta * x.y, im = w * x.y - eta * x.x;
+  for (int m = 0; m < o; ++m) {
+    const double f = Fmi[(long long)m * o + i];
+    const double2 xm = reinterpret_cast<const double2*>(xin + (long long)m * Nc)[r];
+    re -= f * xm.x;
+    im -= f * xm.y;
+  }
+  double2* out = reinterpret_cast<double2*>(sout + (long long)i * Nc) + r;
+  double2 cur = *out;
+  cur.x += re;
+  cur.y += im;
+  *out = cur;
+}
+
+// sigma2 epilogue: s2[(i<j)][a][c] += (w - i eta) x2 + Z[i][a][j][c] - Z[j][a][i][c]
+__global__ void k_sigma2_epilogue(double* __restrict__ sout, const double* __restrict__ xin, const double* __restrict__ Z,
+                                  const double* __restrict__ omega, double eta, int o, int v, int nrhs) {
+  // blockIdx.x = pair*v + a ; threads over r
+  const long long row = blockIdx.x;
+  const long long pr = row / v;
+  const int a = row % v;
+  int i, j;
+  decode_pair(pr, o, i, j);
+  const int Nc = 2 * nrhs;
+  const double2* x = reinterpret_cast<const double2*>(xin + ((long long)o + row) * Nc);
+  double2* s = reinterpret_cast<double2*>(sout + ((long long)o + row) * Nc);
+  const double2* zij = reinterpret_cast<const double2*>(Z + (((long long)i * v + a) * o + j) * Nc);
+  const double2* zji = reinterpret_cast<const double2*>(Z + (((long long)j * v + a) * o + i) * Nc);
+  for (int r = threadIdx.x; r < nrhs; r += blockDim.x) {
+    const double w = omega[r];
+    const double2 xv = x[r], p = zij[r], q = zji[r];
+    double2 cur = s[r];
+    cur.x += w * xv.x + eta * xv.y + p.x - q.x;
+    cur.y += w * xv.y - eta * xv.x + p.y - q.y;
+    s[r] = cur;
+  }
+}
+
+// ------------------------------------------------------------------------------------
+// GMRES building blocks on vec[n][Nc] matrices (complex columns = double2 per rhs)
+// ------------------------------------------------------------------------------------
+// partial[blk][k][r] = sum over this block's rows of conj(V_k[row][r]) * w[row][r],  k in [0,nk), nk <= NK.
+// blockDim = (TX rhs lanes, TY row lanes); gridDim = (row blocks, ceil(nrhs/TX)); dynamic smem TX*TY double2.
+template <int NK>
+__global__ void k_multi_dot(double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
+                            long long n, int nrhs, int nk) {
+  extern __shared__ double2 sred[];
+  double2 acc[NK];
+#pragma unroll
+  for (int k = 0; k < NK; ++k) acc[k] = make_double2(0.0, 0.0);
+  const long long rows_per_block = (n + gridDim.x - 1) / gridDim.x;
+  const long long rbeg = (long long)blockIdx.x * rows_per_block;
+  const long long rend = min(n, rbeg + rows_per_block);
+  const int r = blockIdx.y * blockDim.x + threadIdx.x;
+  const bool ok = r < nrhs;
+  if (ok) {
+    for (long long row = rbeg + threadIdx.y; row < rend; row += blockDim.y) {
+      const double2 wv = reinterpret_cast<const double2*>(w)[row * nrhs + r];
+#pragma unroll
+      for (int k = 0; k < NK; ++k)
+        if (k < nk) {
+          const double2 vv = reinterpret_cast<const double2*>(Vs[k])[row * nrhs + r];
+          acc[k].x += vv.x * wv.x + vv.y * wv.y;   // conj(v) * w
+          acc[k].y += vv.x * wv.y - vv.y * wv.x;
+        }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < NK; ++k) {
+    if (k < nk) {   // nk is block-uniform
+      sred[threadIdx.y * blockDim.x + threadIdx.x] = acc[k];
+      __syncthreads();
+      if (threadIdx.y == 0 && ok) {
+        double2 s = sred[threadIdx.x];
+        for (int yy = 1; yy < blockDim.y; ++yy) {
+          const double2 t = sred[yy * blockDim.x + threadIdx.x];
+          s.x += t.x;
+          s.y += t.y;
+        }
+        partial[((long long)blockIdx.x * nk + k) * nrhs + r] = s;
+      }
+      __syncthreads();
+    }
+  }
+}
+// h[k][r] (+)= sum_blk partial[blk][k][r]
+__global__ void k_dot_finish(double2* __restrict__ h, const double2* __restrict__ partial, int nblk, int nk, int nrhs,
+                             int accumulate) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nk * nrhs) return;
+  double2 s = make_double2(0.0, 0.0);
+  for (int b = 0; b < nblk; ++b) {
+    const double2 t = partial[(long long)b * nk * nrhs + idx];
+    s.x += t.x;
+    s.y += t.y;
+  }
+  if (accumulate) { s.x += h[idx].x; s.y += h[idx].y; }
+  h[idx] = s;
+}
+// w[row][r] += sign * sum_k coef[k][r] * V_k[row][r]     (nk <= NK per launch)
+template <int NK>
+__global__ void k_multi_axpy(double* __restrict__ w, const double* const* __restrict__ Vs, const double2* __restrict__ coef,
+                             long long n, int nrhs, int nk, double sign) {
+  const long long total = n * nrhs;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const long long row = idx / nrhs;
+    const int r = idx % nrhs;
+    double2 acc = reinterpret_cast<double2*>(w)[idx];
+#pragma unroll
+    for (int k = 0; k < NK; ++k)
+      if (k < nk) {
+        const double2 c = coef[(long long)k * nrhs + r];
+        const double2 vv = reinterpret_cast<const double2*>(Vs[k])[row * nrhs + r];
+        acc.x += sign * (c.x * vv.x - c.y * vv.y);
+        acc.y += sign * (c.x * vv.y + c.y * vv.x);
+      }
+    reinterpret_cast<double2*>(w)[idx] = acc;
+  }
+}
+// out[row][r] = scale[r] * in[row][r]   (real scale per rhs; scale 0 masks a converged / broken-down column)
+__global__ void k_scale_cols(double* __restrict__ out, const double* __restrict__ in, const double* __restrict__ scale,
+                             long long n, int nrhs) {
+  const long long total = n * nrhs;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const int r = idx % nrhs;
+    const double s = scale[r];
+    double2 x = reinterpret_cast<const double2*>(in)[idx];
+    x.x *= s;
+    x.y *= s;
+    reinterpret_cast<double2*>(out)[idx] = x;
+  }
+}
+// a[k] += b[k] (complex arrays)
+__global__ void k_cadd(double2* __restrict__ a, const double2* __restrict__ b, int n) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n) { a[idx].x += b[idx].x; a[idx].y += b[idx].y; }
+}
+// r = b - Ax
+__global__ void k_residual(double* __restrict__ r, const double* __restrict__ b, const double* __restrict__ ax, long long n2) {
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n2; idx += (long long)gridDim.x * blockDim.x)
+    r[idx] = b[idx] - ax[idx];
+}
+
+}  // namespace gfcc

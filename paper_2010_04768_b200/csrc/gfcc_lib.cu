@@ -1,0 +1,899 @@
+// =====================================================================================
+// gfcc_lib.cu -- C ABI of the B200-native GFCCSD-IP hot path (see include/gfcc.h).
+//
+//   gfcc_create   : SURVEY.md 8a P1-P7  (one-time intermediates)
+//   gfcc_sigma_ip : SURVEY.md 8a S1-S13 (batched sigma, Eq. 5, Alg. 1)
+//   gfcc_solve_ip : SURVEY.md 8a G1-G6  (batched GMRES PAPER.md:136-138 + G assembly PAPER.md:89-94)
+//
+// Every O(N^5)/O(N^6) contraction is a real FP64 GEMM on the DMMA engine of gfcc_gemm.cuh with the RHS
+// batch folded into N; the (ov x ov) ring/exchange integrals are streamed through bounded panels built
+// on the fly from the Cholesky vectors (never stored; BASELINE.json configs[2..4]).  No CPU fallback.
+// =====================================================================================
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#include <algorithm>
+
+#include "../../include/gfcc.h"
+#include "gfcc_gemm.cuh"
+#include "gfcc_kernels.cuh"
+#include "gfcc_solve.cuh"
+
+using namespace gfcc;
+
+static thread_local std::string g_create_error;
+
+struct gfcc_ctx {
+  int o = 0, v = 0, Q = 0, N = 0;
+  long long npair = 0, ntri = 0, nvec = 0;   // nvec = o + npair*v (rows of an internal vector)
+  cudaStream_t stream = 0;
+  std::string err;
+  std::vector<void*> allocs;
+  double bytes = 0;
+  // ---- intermediates (device) ----
+  double *Lov = nullptr, *LooT = nullptr, *Lvv = nullptr, *Lm = nullptr;   // [Q][o][v], [Q][i][m], [Q][a][e], [Q][i][a]
+  double *Fme = nullptr, *Fmi = nullptr, *Fae = nullptr, *fdiag = nullptr;
+  double *Wp = nullptr;    // W_mnij  packed [(i<j)][(m<n)]
+  double *WB = nullptr;    // W_mbij  packed [(i<j)][a][m] = W[m,a,j,i]
+  double *D = nullptr, *t1 = nullptr, *l1 = nullptr;
+  const double *T2p = nullptr, *L2p = nullptr;   // borrowed
+  long long* blk_tab = nullptr;   // [o][o] element offset of the T2 block of the pair {i,n}
+  double* blk_sgn = nullptr;      // [o][o] +1 (i<n), -1 (i>n), 0 (i==n)
+  // ---- workspace, sized for ws_nrhs ----
+  int ws_nrhs = 0;
+  double *XU = nullptr, *Z = nullptr, *V = nullptr, *Y = nullptr, *KP = nullptr, *yv = nullptr, *part = nullptr, *d_omega = nullptr;
+  double *vin = nullptr, *vout = nullptr;   // internal vectors for gfcc_sigma_ip
+  long long part_elems = 0;
+  int panel_ni = 1;
+  // ---- options / stats ----
+  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3e9, opt_max_batch = 256;
+  double st_iterations = 0, st_sigma_apps = 0, st_flops_sigma = 0, st_flops_create = 0, st_max_relres = 0, st_nunconv = 0;
+  double st_gemm_launches = 0, st_kernel_launches = 0, st_flops_exec = 0;
+  std::vector<double> last_relres;
+  std::vector<int> last_iters;
+  SolveWs sw;
+};
+
+#define CUDA_TRY(h, expr)                                                                      \
+  do {                                                                                         \
+    cudaError_t e__ = (expr);                                                                  \
+    if (e__ != cudaSuccess) {                                                                  \
+      char buf__[512];                                                                         \
+      snprintf(buf__, sizeof buf__, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+      (h)->err = buf__;                                                                        \
+      return (e__ == cudaErrorMemoryAllocation) ? GFCC_ENOMEM : GFCC_ECUDA;                    \
+    }                                                                                          \
+  } while (0)
+#define TRY(expr) do { int rc__ = (expr); if (rc__ != GFCC_OK) return rc__; } while (0)
+#define KLAUNCH(h) do { (h)->st_kernel_launches += 1; CUDA_TRY(h, cudaGetLastError()); } while (0)
+
+static int dev_alloc(gfcc_ctx* h, double** p, long long elems) {
+  if (elems <= 0) elems = 1;
+  void* q = nullptr;
+  cudaError_t e = cudaMalloc(&q, (size_t)elems * sizeof(double));
+  if (e != cudaSuccess) {
+    char buf[256];
+    snprintf(buf, sizeof buf, "cudaMalloc of %.3f GB failed: %s", elems * 8e-9, cudaGetErrorString(e));
+    h->err = buf;
+    cudaGetLastError();
+    return GFCC_ENOMEM;
+  }
+  h->allocs.push_back(q);
+  h->bytes += (double)elems * 8;
+  *p = (double*)q;
+  return GFCC_OK;
+}
+static void dev_free(gfcc_ctx* h, double* p, long long elems) {
+  if (!p) return;
+  for (size_t k = 0; k < h->allocs.size(); ++k)
+    if (h->allocs[k] == (void*)p) { h->allocs.erase(h->allocs.begin() + k); break; }
+  cudaFree(p);
+  h->bytes -= (double)std::max(elems, 1LL) * 8;
+}
+
+static int gemm(gfcc_ctx* h, const GemmDesc& d) {
+  CUDA_TRY(h, launch_dgemm(d, h->stream));
+  h->st_gemm_launches += 1;
+  h->st_kernel_launches += 1;
+  h->st_flops_exec += 2.0 * d.M * (double)d.N * (double)d.K1 * d.K0 * d.batch;
+  return GFCC_OK;
+}
+
+// split the K1 blocks of a GEMM over S batches, partial sums in h->part, deterministic reduction
+static int gemm_splitk(gfcc_ctx* h, GemmDesc d, int S) {
+  S = std::max(1, std::min(S, d.K1));
+  const long long need = (long long)S * d.M * d.N;
+  if (S == 1 || d.batch != 1 || d.tabA || d.tabB || d.sgn || need > h->part_elems) return gemm(h, d);
+  const int chunk = (d.K1 + S - 1) / S;
+  // K1 blocks [z*chunk, min(K1,(z+1)*chunk)): launch full chunks as one batched GEMM, the ragged tail separately
+  const int full = d.K1 / chunk;            // batches with exactly `chunk` blocks
+  const int tail = d.K1 - full * chunk;     // blocks in the last partial batch
+  GemmDesc g = d;
+  g.C = h->part; g.sCm0 = d.N; g.sCm1 = 0; g.Md = d.M; g.sCn0 = 1; g.sCn1 = 0; g.Nd = d.N;
+  g.alpha = 1.0; g.beta = 0.0;
+  g.K1 = chunk; g.batch = full;
+  g.bsA = (long long)chunk * d.sAk1; g.bsB = (long long)chunk * d.sBk1; g.bsC = (long long)d.M * d.N;
+  if (full > 0) TRY(gemm(h, g));
+  int nparts = full;
+  if (tail > 0) {
+    GemmDesc t = g;
+    t.K1 = tail; t.batch = 1;
+    t.A = d.A + (long long)full * chunk * d.sAk1;
+    t.B = d.B + (long long)full * chunk * d.sBk1;
+    t.C = h->part + (long long)full * d.M * d.N;
+    TRY(gemm(h, t));
+    ++nparts;
+  }
+  const long long tot = (long long)d.M * d.N;
+  k_splitk_reduce<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(d.C, h->part, nparts, d.M, d.N, d.alpha, d.beta, d.sCm0,
+                                                                      d.sCm1, d.Md > 0 ? d.Md : d.M, d.sCn0, d.sCn1,
+                                                                      d.Nd > 0 ? d.Nd : d.N);
+  KLAUNCH(h);
+  return GFCC_OK;
+}
+
+static inline unsigned nblk(long long n, int t = 256, long long cap = 148LL * 32) {
+  long long b = (n + t - 1) / t;
+  return (unsigned)std::max(1LL, std::min(b, cap));
+}
+
+// ------------------------------------------------------------------------------------------
+// workspace for a batch of nrhs right-hand sides
+// ------------------------------------------------------------------------------------------
+static void free_workspace(gfcc_ctx* h) {
+  const int o = h->o, v = h->v;
+  const long long Nc = 2LL * h->ws_nrhs, big = (long long)o * v * o * Nc;
+  dev_free(h, h->XU, big); dev_free(h, h->Z, big); dev_free(h, h->V, big);
+  dev_free(h, h->Y, (long long)h->Q * o * Nc);
+  dev_free(h, h->KP, (long long)h->panel_ni * v * o * v);
+  dev_free(h, h->yv, (long long)v * Nc);
+  dev_free(h, h->d_omega, h->ws_nrhs);
+  dev_free(h, h->vin, h->nvec * Nc); dev_free(h, h->vout, h->nvec * Nc);
+  h->XU = h->Z = h->V = h->Y = h->KP = h->yv = h->d_omega = h->vin = h->vout = nullptr;
+  h->ws_nrhs = 0;
+}
+
+// choose how many occupied indices one (ov x ov) panel covers: as many as the byte budget allows, preferring
+// counts whose consuming GEMM fills whole waves of 148 CTAs.
+static int choose_panel(int o, int v, long long ncols, double budget_bytes) {
+  const double row_bytes = (double)o * v * 8.0;
+  int nmax = (int)std::min<double>(o, std::floor(budget_bytes / (row_bytes * v)));
+  if (nmax < 1) nmax = 1;
+  int best = nmax; double best_eff = -1;
+  const int tiles_n = (int)((ncols + GEMM_BN - 1) / GEMM_BN);
+  for (int n = nmax; n >= std::max(1, nmax / 2); --n) {
+    const int rows = n * v;
+    const int bm = 16 * pick_wmf(rows);
+    const long long tiles = (long long)((rows + bm - 1) / bm) * tiles_n;
+    const long long waves = (tiles + 147) / 148;
+    const double eff = (double)rows * ncols / ((double)waves * 148 * bm * GEMM_BN);
+    if (eff > best_eff + 1e-9) { best_eff = eff; best = n; }
+  }
+  return best;
+}
+
+static int ensure_workspace(gfcc_ctx* h, int nrhs, bool need_abi_vecs) {
+  const int o = h->o, v = h->v, Q = h->Q;
+  if (h->ws_nrhs != nrhs) {
+    if (h->ws_nrhs) free_workspace(h);
+    const long long Nc = 2LL * nrhs, big = (long long)o * v * o * Nc;
+    h->panel_ni = choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes);
+    h->ws_nrhs = nrhs;
+    TRY(dev_alloc(h, &h->XU, big)); TRY(dev_alloc(h, &h->Z, big)); TRY(dev_alloc(h, &h->V, big));
+    TRY(dev_alloc(h, &h->Y, (long long)Q * o * Nc));
+    TRY(dev_alloc(h, &h->KP, (long long)h->panel_ni * v * o * v));
+    TRY(dev_alloc(h, &h->yv, (long long)v * Nc));
+    TRY(dev_alloc(h, &h->d_omega, nrhs));
+  }
+  if (need_abi_vecs && !h->vin) {
+    const long long Nc = 2LL * nrhs;
+    TRY(dev_alloc(h, &h->vin, h->nvec * Nc));
+    TRY(dev_alloc(h, &h->vout, h->nvec * Nc));
+  }
+  return GFCC_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// sigma on internal vectors:  sout = (omega - i eta) xin + Hbar xin
+// d_omega: device [nrhs].  xin, sout: [nvec][Nc].
+// ------------------------------------------------------------------------------------------
+static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double eta, const double* xin, double* sout) {
+  const int o = h->o, v = h->v, Q = h->Q;
+  const long long Nc = 2LL * nrhs, ld = (long long)o * Nc, ov = (long long)o * v;
+  cudaStream_t st = h->stream;
+  const double* x2 = xin + (long long)o * Nc;
+  double* s2 = sout + (long long)o * Nc;
+
+  // XU[m][e][j][c] = x2[m,j,e]
+  k_unpack_xu<<<(unsigned)ov, 256, 0, st>>>(h->XU, xin, o, v, (int)Nc);
+  KLAUNCH(h);
+  // S1: Y[Q][(j,c)] = sum_(m,e) Lov[Q][(m,e)] XU[(m,e)][(j,c)]
+  {
+    GemmDesc d; d.M = Q; d.N = (int)ld; d.K0 = (int)ov;
+    d.A = h->Lov; d.sAm = ov; d.sAk0 = 1;
+    d.B = h->XU; d.sBk0 = ld; d.sBn = 1;
+    d.C = h->Y; d.sCm0 = ld;
+    TRY(gemm(h, d));
+  }
+  // S7: Z[(i,a)][(j,c)] = sum_Q Lm[Q][(i,a)] Y[Q][(j,c)]
+  {
+    GemmDesc d; d.M = (int)ov; d.N = (int)ld; d.K0 = Q;
+    d.A = h->Lm; d.sAm = 1; d.sAk0 = ov;
+    d.B = h->Y; d.sBk0 = ld; d.sBn = 1;
+    d.C = h->Z; d.sCm0 = ld;
+    TRY(gemm(h, d));
+  }
+  // S8+S9 (+S3,S4 folded): panels of K2'[(i,a)][(m,e)], Z -= K2' XU
+  for (int i0 = 0; i0 < o; i0 += h->panel_ni) {
+    const int ni = std::min(h->panel_ni, o - i0);
+    {
+      GemmDesc d; d.M = ni * o; d.N = v * v; d.K0 = Q;
+      d.A = h->LooT + (long long)i0 * o; d.sAm = 1; d.sAk0 = (long long)o * o;
+      d.B = h->Lvv; d.sBk0 = (long long)v * v; d.sBn = 1;
+      d.C = h->KP; d.Md = o; d.sCm1 = (long long)v * ov; d.sCm0 = v; d.Nd = v; d.sCn1 = ov; d.sCn0 = 1;
+      TRY(gemm(h, d));
+    }
+    k_k2_fixup<<<(unsigned)(ni * v), 128, 0, st>>>(h->KP, h->Fmi, h->Fae, o, v, i0);
+    KLAUNCH(h);
+    {
+      GemmDesc d; d.M = ni * v; d.N = (int)ld; d.K0 = (int)ov;
+      d.A = h->KP; d.sAm = ov; d.sAk0 = 1;
+      d.B = h->XU; d.sBk0 = ld; d.sBn = 1;
+      d.C = h->Z + (long long)i0 * v * ld; d.sCm0 = ld;
+      d.alpha = -1.0; d.beta = 1.0;
+      TRY(gemm(h, d));
+    }
+  }
+  // S10: panels of K4[(n,f)][(m,e)] = sum_Q L[Q,m,f] L[Q,n,e];  V = K4 XU
+  for (int n0 = 0; n0 < o; n0 += h->panel_ni) {
+    const int nn = std::min(h->panel_ni, o - n0);
+    {
+      GemmDesc d; d.M = (int)ov; d.N = nn * v; d.K0 = Q;
+      d.A = h->Lov; d.sAm = 1; d.sAk0 = ov;
+      d.B = h->Lov + (long long)n0 * v; d.sBk0 = ov; d.sBn = 1;
+      d.C = h->KP; d.Md = v; d.sCm1 = v; d.sCm0 = ov; d.Nd = v; d.sCn1 = (long long)v * ov; d.sCn0 = 1;
+      TRY(gemm(h, d));
+    }
+    {
+      GemmDesc d; d.M = nn * v; d.N = (int)ld; d.K0 = (int)ov;
+      d.A = h->KP; d.sAm = ov; d.sAk0 = 1;
+      d.B = h->XU; d.sBk0 = ld; d.sBn = 1;
+      d.C = h->V + (long long)n0 * v * ld; d.sCm0 = ld;
+      TRY(gemm(h, d));
+    }
+  }
+  // S11: Z[i][a][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]   (T2 blocks through the pair table, sign per block)
+  {
+    GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
+    d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
+    d.tabs_even = ((long long)v * v) % 2 == 0;
+    d.B = h->V; d.sBk1 = (long long)v * ld; d.sBk0 = ld; d.sBn = 1;
+    d.C = h->Z; d.sCm0 = ld; d.bsC = (long long)v * ld;
+    d.batch = o; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  // S12a: yv[e][c] = - sum_(Q,m) Lov[Q][m][e] Y[Q][m][c]
+  {
+    GemmDesc d; d.M = v; d.N = (int)Nc; d.K1 = Q; d.K0 = o;
+    d.A = h->Lov; d.sAm = 1; d.sAk0 = v; d.sAk1 = ov;
+    d.B = h->Y; d.sBk0 = Nc; d.sBk1 = ld; d.sBn = 1;
+    d.C = h->yv; d.sCm0 = Nc; d.alpha = -1.0;
+    TRY(gemm_splitk(h, d, 64));
+  }
+  // S2: sigma1[i][c] = sum_(Q,n) Loo[Q,n,i] Y[Q][n][c]  -  sum_(m,e) Fme[m,e] XU[(m,e)][(i,c)]  + small terms
+  {
+    GemmDesc d; d.M = o; d.N = (int)Nc; d.K1 = Q; d.K0 = o;
+    d.A = h->LooT; d.sAm = o; d.sAk0 = 1; d.sAk1 = (long long)o * o;
+    d.B = h->Y; d.sBk0 = Nc; d.sBk1 = ld; d.sBn = 1;
+    d.C = sout; d.sCm0 = Nc;
+    TRY(gemm_splitk(h, d, 64));
+  }
+  {
+    // treat the (m,e) sum as K1 = o blocks of K0 = v so that it can be split
+    GemmDesc d; d.M = 1; d.N = (int)ld; d.K1 = o; d.K0 = v;
+    d.A = h->Fme; d.sAm = ov; d.sAk0 = 1; d.sAk1 = v;
+    d.B = h->XU; d.sBk0 = ld; d.sBk1 = (long long)v * ld; d.sBn = 1;
+    d.C = sout; d.sCm0 = ld; d.alpha = -1.0; d.beta = 1.0;
+    TRY(gemm_splitk(h, d, 32));
+  }
+  k_sigma1_small<<<(unsigned)((o * nrhs + 127) / 128), 128, 0, st>>>(sout, xin, h->Fmi, d_omega, eta, o, nrhs);
+  KLAUNCH(h);
+  // S6 (D): s2[(i<j)][(a,c)] = sum_(m<n) W[(i<j)][(m<n)] x2[(m<n)][(a,c)]
+  {
+    GemmDesc d; d.M = (int)h->npair; d.N = (int)(v * Nc); d.K0 = (int)h->npair;
+    d.A = h->Wp; d.sAm = h->npair; d.sAk0 = 1;
+    d.B = x2; d.sBk0 = v * Nc; d.sBn = 1;
+    d.C = s2; d.sCm0 = v * Nc;
+    TRY(gemm(h, d));
+  }
+  // S12b (F): s2[(pair,a)][c] += sum_e t[(pair),a,e] yv[e][c]
+  {
+    GemmDesc d; d.M = (int)(h->npair * v); d.N = (int)Nc; d.K0 = v;
+    d.A = h->T2p; d.sAm = v; d.sAk0 = 1;
+    d.B = h->yv; d.sBk0 = Nc; d.sBn = 1;
+    d.C = s2; d.sCm0 = Nc; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  // S5 (C): s2[(pair,a)][c] += sum_m WB[(pair,a)][m] x1[m][c]
+  {
+    GemmDesc d; d.M = (int)(h->npair * v); d.N = (int)Nc; d.K0 = o;
+    d.A = h->WB; d.sAm = o; d.sAk0 = 1;
+    d.B = xin; d.sBk0 = Nc; d.sBn = 1;
+    d.C = s2; d.sCm0 = Nc; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  // S13: shift + P(ij) ring
+  k_sigma2_epilogue<<<(unsigned)(h->npair * v), 64, 0, st>>>(sout, xin, h->Z, d_omega, eta, o, v, nrhs);
+  KLAUNCH(h);
+  h->st_sigma_apps += 1;
+  return GFCC_OK;
+}
+
+// executed FP64 flop model of one batched sigma application (GEMM M*N*K products, pair-packed o^4 term)
+static double sigma_flops(const gfcc_ctx* h, int nrhs) {
+  const double o = h->o, v = h->v, Q = h->Q, Nc = 2.0 * nrhs, ov = o * v, np_ = (double)h->npair;
+  double f = 0;
+  f += 2 * Q * ov * o * Nc * 2;              // S1, S7
+  f += 2 * 2 * Q * ov * ov;                  // S8, S10 panel builds (independent of nrhs)
+  f += 3 * 2 * ov * ov * o * Nc;             // S9, S10 (V), S11
+  f += 2 * np_ * np_ * v * Nc;               // S6, pair-packed
+  f += 2 * np_ * v * v * Nc + 2 * np_ * v * o * Nc;   // S12, S5
+  f += 2 * Q * o * v * Nc + 2 * Q * o * o * Nc + 2 * ov * o * Nc;   // yv, sigma1
+  return f;
+}
+
+// ------------------------------------------------------------------------------------------
+// gfcc_create
+// ------------------------------------------------------------------------------------------
+static int create_impl(gfcc_ctx* h, const double* fock, const double* T1, const double* L1, const double* Lchol) {
+  const int o = h->o, v = h->v, Q = h->Q, N = h->N;
+  const long long ov = (long long)o * v, npair = h->npair, vv = (long long)v * v;
+  cudaStream_t st = h->stream;
+  const double flops0 = h->st_flops_exec;
+
+  TRY(dev_alloc(h, &h->Lov, Q * ov)); TRY(dev_alloc(h, &h->LooT, (long long)Q * o * o));
+  TRY(dev_alloc(h, &h->Lvv, Q * vv)); TRY(dev_alloc(h, &h->Lm, Q * ov));
+  TRY(dev_alloc(h, &h->Fme, ov)); TRY(dev_alloc(h, &h->Fmi, (long long)o * o)); TRY(dev_alloc(h, &h->Fae, vv));
+  TRY(dev_alloc(h, &h->fdiag, N)); TRY(dev_alloc(h, &h->D, (long long)o * o));
+  TRY(dev_alloc(h, &h->t1, ov)); TRY(dev_alloc(h, &h->l1, ov));
+  TRY(dev_alloc(h, &h->Wp, npair * npair)); TRY(dev_alloc(h, &h->WB, npair * v * o));
+  // split-K partial buffer, sized for the largest user
+  h->part_elems = std::max<long long>({64LL * v * 512, 64LL * o * 512, 32LL * o * 512, 32LL * vv, 32LL * o * o, 1LL << 20});
+  TRY(dev_alloc(h, &h->part, h->part_elems));
+  CUDA_TRY(h, cudaMemcpyAsync(h->t1, T1, ov * 8, cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(h, cudaMemcpyAsync(h->l1, L1, ov * 8, cudaMemcpyDeviceToDevice, st));
+  CUDA_TRY(h, cudaMemcpy2DAsync(h->fdiag, 8, fock, (size_t)(N + 1) * 8, 8, N, cudaMemcpyDeviceToDevice, st));
+  {   // pair-block table for the T2 operand
+    std::vector<long long> tab((size_t)o * o, 0);
+    std::vector<double> sg((size_t)o * o, 0.0);
+    for (int i = 0; i < o; ++i)
+      for (int n = 0; n < o; ++n) {
+        if (i == n) continue;
+        tab[(size_t)i * o + n] = pair_index(std::min(i, n), std::max(i, n), o) * vv;
+        sg[(size_t)i * o + n] = (i < n) ? 1.0 : -1.0;
+      }
+    double* tmp = nullptr;
+    TRY(dev_alloc(h, &tmp, (long long)o * o)); h->blk_tab = (long long*)tmp;
+    TRY(dev_alloc(h, &h->blk_sgn, (long long)o * o));
+    CUDA_TRY(h, cudaMemcpyAsync(h->blk_tab, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(h, cudaMemcpyAsync(h->blk_sgn, sg.data(), sg.size() * 8, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(h, cudaStreamSynchronize(st));   // host vectors go out of scope
+  }
+  auto copy_block = [&](double* dst, int R, int Cc, int row0, int col0, int transpose) {
+    dim3 grid((Cc + 31) / 32, (R + 31) / 32, Q), blk(32, 8);
+    k_copy_block<<<grid, blk, 0, st>>>(dst, Lchol, R, Cc, row0, col0, N, transpose);
+  };
+  // ---- P1: T1-dressed Cholesky blocks ----
+  copy_block(h->Lov, o, v, 0, o, 0); KLAUNCH(h);          // Lov[Q][m][e] = L[Q][m][o+e]
+  copy_block(h->LooT, o, o, 0, 0, 1); KLAUNCH(h);         // LooT[Q][i][m] = L[Q][m][i]
+  copy_block(h->Lvv, v, v, o, o, 0); KLAUNCH(h);          // Lvv[Q][a][e] = L[Q][o+a][o+e]
+  copy_block(h->Lm, o, v, o, 0, 1); KLAUNCH(h);           // Lm[Q][i][a] = L[Q][o+a][i]
+  {   // LooT[Q][i][m] += sum_e t1[i,e] Lov[Q][m][e]
+    GemmDesc d; d.M = o; d.N = o; d.K0 = v; d.batch = Q;
+    d.A = h->t1; d.sAm = v; d.sAk0 = 1;
+    d.B = h->Lov; d.sBk0 = 1; d.sBn = v; d.bsB = ov;
+    d.C = h->LooT; d.sCm0 = o; d.bsC = (long long)o * o; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  {   // Lm[Q][i][a] -= sum_m L[Q][m][i] t1[m,a]      (uses the UNdressed L_mi)
+    GemmDesc d; d.M = o; d.N = v; d.K0 = o; d.batch = Q;
+    d.A = Lchol; d.sAm = 1; d.sAk0 = N; d.bsA = (long long)N * N;
+    d.B = h->t1; d.sBk0 = v; d.sBn = 1;
+    d.C = h->Lm; d.sCm0 = v; d.bsC = ov; d.alpha = -1.0; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  {   // Lvv[Q][a][e] -= sum_m t1[m,a] Lov[Q][m][e]
+    GemmDesc d; d.M = v; d.N = v; d.K0 = o; d.batch = Q;
+    d.A = h->t1; d.sAm = 1; d.sAk0 = v;
+    d.B = h->Lov; d.sBk0 = v; d.sBn = 1; d.bsB = ov;
+    d.C = h->Lvv; d.sCm0 = v; d.bsC = vv; d.alpha = -1.0; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  {   // Lm[Q][i][a] += sum_e t1[i,e] Lvv[Q][a][e]     (dressed Lvv)  -> Lm holds Ltilde_vo[Q,a,i]
+    GemmDesc d; d.M = o; d.N = v; d.K0 = v; d.batch = Q;
+    d.A = h->t1; d.sAm = v; d.sAk0 = 1;
+    d.B = h->Lvv; d.sBk0 = 1; d.sBn = v; d.bsB = vv;
+    d.C = h->Lm; d.sCm0 = v; d.bsC = ov; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
+  // ---- P2: dressed Fock  ft = A^T (f + J - K) B ----
+  double *sq = nullptr, *U = nullptr, *Kmat = nullptr, *g = nullptr, *tmp = nullptr, *ft = nullptr;
+  TRY(dev_alloc(h, &sq, Q)); TRY(dev_alloc(h, &U, (long long)Q * N * o));
+  TRY(dev_alloc(h, &Kmat, (long long)N * N)); TRY(dev_alloc(h, &g, (long long)N * N));
+  TRY(dev_alloc(h, &tmp, (long long)N * N)); TRY(dev_alloc(h, &ft, (long long)N * N));
+  k_sq<<<Q, 256, 0, st>>>(sq, h->t1, h->Lov, (int)ov); KLAUNCH(h);
+  {   // U[Q][p][k] = sum_c L[Q][p][o+c] t1[k,c]
+    GemmDesc d; d.M = N; d.N = o; d.K0 = v; d.batch = Q;
+    d.A = Lchol + o; d.sAm = N; d.sAk0 = 1; d.bsA = (long long)N * N;
+    d.B = h->t1; d.sBk0 = 1; d.sBn = v;
+    d.C = U; d.sCm0 = o; d.bsC = (long long)N * o;
+    TRY(gemm(h, d));
+  }
+  {   // K[p][q] = sum_(Q,k) U[Q][p][k] L[Q][k][q]
+    GemmDesc d; d.M = N; d.N = N; d.K1 = Q; d.K0 = o;
+    d.A = U; d.sAm = o; d.sAk0 = 1; d.sAk1 = (long long)N * o;
+    d.B = Lchol; d.sBk0 = N; d.sBk1 = (long long)N * N; d.sBn = 1;
+    d.C = Kmat; d.sCm0 = N;
+    const int S = (int)std::max<long long>(1, std::min<long long>(32, h->part_elems / ((long long)N * N)));
+    TRY(gemm_splitk(h, d, S));
+  }
+  k_fock_jk<<<(unsigned)(((long long)N * N + 127) / 128), 128, 0, st>>>(g, fock, sq, Lchol, Kmat, N, Q); KLAUNCH(h);
+  k_dress_left<<<(unsigned)(((long long)N * N + 127) / 128), 128, 0, st>>>(tmp, g, h->t1, o, v); KLAUNCH(h);
+  k_dress_right<<<(unsigned)(((long long)N * N + 127) / 128), 128, 0, st>>>(ft, tmp, h->t1, o, v); KLAUNCH(h);
+  k_fock_block<<<(unsigned)((ov + 127) / 128), 128, 0, st>>>(h->Fme, ft, o, v, 0, o, N); KLAUNCH(h);
+  k_fock_block<<<(unsigned)(((long long)o * o + 127) / 128), 128, 0, st>>>(h->Fmi, ft, o, o, 0, 0, N); KLAUNCH(h);
+  k_fock_block<<<(unsigned)((vv + 127) / 128), 128, 0, st>>>(h->Fae, ft, v, v, o, o, N); KLAUNCH(h);
+  CUDA_TRY(h, cudaStreamSynchronize(st));
+  dev_free(h, sq, Q); dev_free(h, U, (long long)Q * N * o); dev_free(h, Kmat, (long long)N * N);
+  dev_free(h, g, (long long)N * N); dev_free(h, tmp, (long long)N * N); dev_free(h, ft, (long long)N * N);
+
+  // ---- P3: Mq[Q][i][a] = sum_(n,f) t[i,n,f,a] Lov[Q][n][f]   (batch over i, T2 blocks via the pair table on B)
+  double* Mq = nullptr;
+  TRY(dev_alloc(h, &Mq, Q * ov));
+  {
+    GemmDesc d; d.M = Q; d.N = v; d.K1 = o; d.K0 = v; d.batch = o;
+    d.A = h->Lov; d.sAm = ov; d.sAk0 = 1; d.sAk1 = v;
+    d.B = h->T2p; d.sBk0 = v; d.sBn = 1; d.tabB = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
+    d.tabs_even = (vv % 2) == 0;
+    d.C = Mq; d.sCm0 = ov; d.bsC = v;
+    TRY(gemm(h, d));
+  }
+  // ---- P4: F_mi -= sum_(Q,e) Lov[Q,m,e] M[Q,i,e];  F_ae += sum_(Q,m) M[Q,m,a] Lov[Q,m,e]
+  {
+    GemmDesc d; d.M = o; d.N = o; d.K1 = Q; d.K0 = v;
+    d.A = h->Lov; d.sAm = v; d.sAk0 = 1; d.sAk1 = ov;
+    d.B = Mq; d.sBk0 = 1; d.sBn = v; d.sBk1 = ov;
+    d.C = h->Fmi; d.sCm0 = o; d.alpha = -1.0; d.beta = 1.0;
+    TRY(gemm_splitk(h, d, 32));
+  }
+  {
+    GemmDesc d; d.M = v; d.N = v; d.K1 = Q; d.K0 = o;
+    d.A = Mq; d.sAm = 1; d.sAk0 = v; d.sAk1 = ov;
+    d.B = h->Lov; d.sBk0 = v; d.sBk1 = ov; d.sBn = 1;
+    d.C = h->Fae; d.sCm0 = v; d.alpha = 1.0; d.beta = 1.0;
+    TRY(gemm_splitk(h, d, 32));
+  }
+  // Lm = Ltilde_vo - M
+  k_sub<<<nblk(Q * ov), 256, 0, st>>>(h->Lm, Mq, Q * ov); KLAUNCH(h);
+  CUDA_TRY(h, cudaStreamSynchronize(st));
+  dev_free(h, Mq, Q * ov);
+
+  // ---- create-time panel scratch ----
+  const double budget = h->opt_panel_bytes;
+  // ---- P5: W_mnij packed ----
+  CUDA_TRY(h, cudaMemsetAsync(h->Wp, 0, (size_t)(npair * npair) * 8, st));
+  {
+    // term 1: sum_Q Loo[Q,m,i] Loo[Q,n,j] antisymmetrised in (i,j); panels over i
+    const long long oo = (long long)o * o;
+    int ni = (int)std::max<double>(1, std::min<double>(o, std::floor(budget / (8.0 * o * oo))));
+    double* G1 = nullptr;
+    TRY(dev_alloc(h, &G1, (long long)ni * o * oo));
+    for (int i0 = 0; i0 < o; i0 += ni) {
+      const int n_i = std::min(ni, o - i0);
+      GemmDesc d; d.M = n_i * o; d.N = (int)oo; d.K0 = Q;
+      d.A = h->LooT + (long long)i0 * o; d.sAm = 1; d.sAk0 = oo;
+      d.B = h->LooT; d.sBk0 = oo; d.sBn = 1;
+      d.C = G1; d.sCm0 = oo;
+      TRY(gemm(h, d));
+      for (int mode = 0; mode < 2; ++mode) {
+        k_scatter_oooo<<<nblk((long long)n_i * o * npair), 256, 0, st>>>(h->Wp, G1, o, i0, n_i, mode);
+        KLAUNCH(h);
+      }
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    dev_free(h, G1, (long long)ni * o * oo);
+    // term 2: sum_ef t[i,j,e,f] <mn|ef>, <mn|ef> = sum_Q L[Q,m,e] L[Q,n,f]; panels over m, columns n >= m0 only
+    int nm = (int)std::max<double>(1, std::min<double>(o, std::floor(budget / (8.0 * vv * o))));
+    double *O = nullptr, *tmpw = nullptr;
+    TRY(dev_alloc(h, &O, vv * nm * o)); TRY(dev_alloc(h, &tmpw, npair * nm * o));
+    for (int m0 = 0; m0 < o; m0 += nm) {
+      const int n_m = std::min(nm, o - m0);
+      const int nlo = m0, ncols = o - nlo;       // only n >= m0 can satisfy m < n
+      const long long ldO = (long long)n_m * ncols;
+      {   // O[(e,f)][(m',n')] = sum_Q Lov[Q][(m,e)] Lov[Q][(n,f)]
+        GemmDesc d; d.M = n_m * v; d.N = ncols * v; d.K0 = Q;
+        d.A = h->Lov + (long long)m0 * v; d.sAm = 1; d.sAk0 = ov;
+        d.B = h->Lov + (long long)nlo * v; d.sBk0 = ov; d.sBn = 1;
+        d.C = O; d.Md = v; d.sCm1 = ncols; d.sCm0 = (long long)v * ldO; d.Nd = v; d.sCn1 = 1; d.sCn0 = ldO;
+        TRY(gemm(h, d));
+      }
+      {   // tmpw[(i<j)][(m',n')] = sum_(e,f) T2p[(i<j)][(e,f)] O[(e,f)][(m',n')]
+        GemmDesc d; d.M = (int)npair; d.N = (int)ldO; d.K0 = (int)vv;
+        d.A = h->T2p; d.sAm = vv; d.sAk0 = 1;
+        d.B = O; d.sBk0 = ldO; d.sBn = 1;
+        d.C = tmpw; d.sCm0 = ldO;
+        TRY(gemm(h, d));
+      }
+      k_pack_oooo_cols<<<nblk(npair * ldO), 256, 0, st>>>(h->Wp, tmpw, o, m0, n_m, nlo, 1.0);
+      KLAUNCH(h);
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    dev_free(h, O, vv * nm * o); dev_free(h, tmpw, npair * nm * o);
+  }
+  // ---- P6: W_mbij.  Wacc[(i<j)][b][m] accumulates W[m,b,i,j]; WB = -Wacc (= W[m,b,j,i]) ----
+  CUDA_TRY(h, cudaMemsetAsync(h->WB, 0, (size_t)(npair * v * o) * 8, st));
+  {
+    // term A: P(ij) sum_Q Loo[Q,m,i] Lm[Q,j,b]; panels over i
+    int ni = (int)std::max<double>(1, std::min<double>(o, std::floor(budget / (8.0 * o * ov))));
+    double* X1 = nullptr;
+    TRY(dev_alloc(h, &X1, (long long)ni * o * ov));
+    for (int i0 = 0; i0 < o; i0 += ni) {
+      const int n_i = std::min(ni, o - i0);
+      GemmDesc d; d.M = n_i * o; d.N = (int)ov; d.K0 = Q;
+      d.A = h->LooT + (long long)i0 * o; d.sAm = 1; d.sAk0 = (long long)o * o;
+      d.B = h->Lm; d.sBk0 = ov; d.sBn = 1;
+      d.C = X1; d.sCm0 = ov;
+      TRY(gemm(h, d));
+      for (int mode = 0; mode < 2; ++mode) {
+        k_scatter_ovoo<<<nblk((long long)n_i * o * ov), 256, 0, st>>>(h->WB, X1, o, v, i0, n_i, mode);
+        KLAUNCH(h);
+      }
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    dev_free(h, X1, (long long)ni * o * ov);
+    // term B: - sum_e Fme[m,e] t[i,j,b,e]
+    {
+      GemmDesc d; d.M = (int)(npair * v); d.N = o; d.K0 = v;
+      d.A = h->T2p; d.sAm = v; d.sAk0 = 1;
+      d.B = h->Fme; d.sBk0 = 1; d.sBn = v;
+      d.C = h->WB; d.sCm0 = o; d.alpha = -1.0; d.beta = 1.0;
+      TRY(gemm(h, d));
+    }
+    // term C: sum_(e,f) t[i,j,e,f] R[(e,f)][(b,m)],  R = sum_Q Lov[Q,m,e] Lvv[Q,b,f]; panels over b
+    int nb = (int)std::max<double>(1, std::min<double>(v, std::floor(budget / (8.0 * vv * o))));
+    double* R = nullptr;
+    TRY(dev_alloc(h, &R, vv * nb * o));
+    for (int b0 = 0; b0 < v; b0 += nb) {
+      const int n_b = std::min(nb, v - b0);
+      const long long ldR = (long long)n_b * o;
+      {
+        GemmDesc d; d.M = (int)ov; d.N = n_b * v; d.K0 = Q;
+        d.A = h->Lov; d.sAm = 1; d.sAk0 = ov;
+        d.B = h->Lvv + (long long)b0 * v; d.sBk0 = vv; d.sBn = 1;
+        d.C = R; d.Md = v; d.sCm1 = 1; d.sCm0 = (long long)v * ldR; d.Nd = v; d.sCn1 = o; d.sCn0 = ldR;
+        TRY(gemm(h, d));
+      }
+      {
+        GemmDesc d; d.M = (int)npair; d.N = (int)ldR; d.K0 = (int)vv;
+        d.A = h->T2p; d.sAm = vv; d.sAk0 = 1;
+        d.B = R; d.sBk0 = ldR; d.sBn = 1;
+        d.C = h->WB + (long long)b0 * o; d.sCm0 = (long long)v * o; d.beta = 1.0;
+        TRY(gemm(h, d));
+      }
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    dev_free(h, R, vv * nb * o);
+    // term D: X2[m,b,i,j] = - sum_(n,e) S[(i,m)][(n,e)] t[j,n,b,e],  S = sum_Q Loo[Q,n,i] Lov[Q,m,e]; panels over i
+    int ni2 = (int)std::max<double>(1, std::min<double>(o, std::floor(budget / (8.0 * (o * ov + (double)o * o * v)))));
+    double *S = nullptr, *X2 = nullptr;
+    TRY(dev_alloc(h, &S, (long long)ni2 * o * ov)); TRY(dev_alloc(h, &X2, (long long)o * ni2 * o * v));
+    for (int i0 = 0; i0 < o; i0 += ni2) {
+      const int n_i = std::min(ni2, o - i0);
+      {   // S[(i',m)][(n,e)] : GEMM rows (i',n) from LooT, cols (m,e) from Lov
+        GemmDesc d; d.M = n_i * o; d.N = (int)ov; d.K0 = Q;
+        d.A = h->LooT + (long long)i0 * o; d.sAm = 1; d.sAk0 = (long long)o * o;
+        d.B = h->Lov; d.sBk0 = ov; d.sBn = 1;
+        d.C = S; d.Md = o; d.sCm1 = (long long)o * ov; d.sCm0 = v; d.Nd = v; d.sCn1 = ov; d.sCn0 = 1;
+        TRY(gemm(h, d));
+      }
+      {   // batch j: X2[j][(i',m)][b] = - sum_(n,e) S[(i',m)][(n,e)] sgn(j,n) T2p[blk(j,n)][b][e]
+        GemmDesc d; d.M = n_i * o; d.N = v; d.K1 = o; d.K0 = v; d.batch = o;
+        d.A = S; d.sAm = ov; d.sAk0 = 1; d.sAk1 = v;
+        d.B = h->T2p; d.sBk0 = 1; d.sBn = v; d.tabB = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
+        d.tabs_even = (vv % 2) == 0;
+        d.C = X2; d.sCm0 = v; d.bsC = (long long)n_i * o * v; d.alpha = -1.0;
+        TRY(gemm(h, d));
+      }
+      for (int mode = 0; mode < 2; ++mode) {
+        k_scatter_ovoo_batched<<<nblk((long long)o * n_i * o * v), 256, 0, st>>>(h->WB, X2, o, v, i0, n_i, mode);
+        KLAUNCH(h);
+      }
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    dev_free(h, S, (long long)ni2 * o * ov); dev_free(h, X2, (long long)o * ni2 * o * v);
+    // WB[(i<j)][a][m] = W[m,a,j,i] = -W[m,a,i,j]
+    k_scale<<<nblk(npair * v * o), 256, 0, st>>>(h->WB, -1.0, npair * v * o); KLAUNCH(h);
+  }
+  // ---- P7: D[k][i] = sum_a t1[k,a] l1[i,a] + 1/2 sum_(j,a,b) t[k,j,a,b] l[i,j,a,b] ----
+  {
+    k_D_singles<<<(o * o + 127) / 128, 128, 0, st>>>(h->D, h->t1, h->l1, o, v); KLAUNCH(h);
+    double *TJ = nullptr, *LJ = nullptr;
+    TRY(dev_alloc(h, &TJ, (long long)o * vv)); TRY(dev_alloc(h, &LJ, (long long)o * vv));
+    for (int j = 0; j < o; ++j) {
+      k_gather_t2_rows<<<nblk((long long)o * vv), 256, 0, st>>>(TJ, h->T2p, o, v, j); KLAUNCH(h);
+      k_gather_l2_rows<<<nblk((long long)o * vv), 256, 0, st>>>(LJ, h->L2p, o, v, j); KLAUNCH(h);
+      GemmDesc d; d.M = o; d.N = o; d.K1 = v; d.K0 = v;
+      d.A = TJ; d.sAm = vv; d.sAk0 = 1; d.sAk1 = v;
+      d.B = LJ; d.sBk0 = 1; d.sBn = vv; d.sBk1 = v;
+      d.C = h->D; d.sCm0 = o; d.alpha = 0.5; d.beta = 1.0;
+      TRY(gemm_splitk(h, d, 32));
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    dev_free(h, TJ, (long long)o * vv); dev_free(h, LJ, (long long)o * vv);
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(st));
+  h->st_flops_create = h->st_flops_exec - flops0;
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_create(int o, int v, int Q, const double* fock, const double* T1, const double* T2, const double* L1,
+                           const double* L2, const double* Lchol, gfcc_handle* out) {
+  if (out) *out = nullptr;
+  if (!out || !fock || !T1 || !T2 || !L1 || !L2 || !Lchol || o < 2 || v < 2 || Q < 1) {
+    g_create_error = "gfcc_create: null pointer or invalid size (need o >= 2, v >= 2, Q >= 1)";
+    return GFCC_EINVAL;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    g_create_error = "gfcc_create: no CUDA device (there is no CPU fallback)";
+    cudaGetLastError();
+    return GFCC_ECUDA;
+  }
+  gfcc_ctx* h = new gfcc_ctx();
+  h->o = o; h->v = v; h->Q = Q; h->N = o + v;
+  h->npair = (long long)o * (o - 1) / 2; h->ntri = (long long)v * (v - 1) / 2;
+  h->nvec = o + h->npair * v;
+  h->T2p = T2; h->L2p = L2;
+  int rc = create_impl(h, fock, T1, L1, Lchol);
+  if (rc != GFCC_OK) {
+    g_create_error = h->err;
+    for (void* p : h->allocs) cudaFree(p);
+    delete h;
+    return rc;
+  }
+  *out = h;
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_destroy(gfcc_handle h) {
+  if (!h) return GFCC_EINVAL;
+  cudaStreamSynchronize(h->stream);
+  solve_free(h->sw);
+  for (void* p : h->allocs) cudaFree(p);
+  delete h;
+  return GFCC_OK;
+}
+
+extern "C" const char* gfcc_last_error(gfcc_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+extern "C" int gfcc_set_stream(gfcc_handle h, void* s) {
+  if (!h) return GFCC_EINVAL;
+  h->stream = (cudaStream_t)s;
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
+  if (!h || !key) return GFCC_EINVAL;
+  std::string k(key);
+  if (k == "gmres_m" && val >= 1) h->opt_m = std::floor(val);
+  else if (k == "gmres_maxit" && val >= 1) h->opt_maxit = std::floor(val);
+  else if (k == "gmres_fixed" && val >= 0) h->opt_fixed = std::floor(val);
+  else if (k == "x0" && (val == 0 || val == 1)) h->opt_x0 = val;
+  else if (k == "panel_bytes" && val > 0) { h->opt_panel_bytes = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
+  else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
+  else { h->err = "gfcc_set_option: unknown key or invalid value: " + k; return GFCC_EINVAL; }
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
+  if (!h || !key || !val) return GFCC_EINVAL;
+  std::string k(key);
+  if (k == "iterations") *val = h->st_iterations;
+  else if (k == "sigma_applications") *val = h->st_sigma_apps;
+  else if (k == "flops_sigma") *val = h->st_flops_sigma;
+  else if (k == "flops_create") *val = h->st_flops_create;
+  else if (k == "flops_executed") *val = h->st_flops_exec;
+  else if (k == "bytes_device") *val = h->bytes + h->sw.bytes;
+  else if (k == "max_relres") *val = h->st_max_relres;
+  else if (k == "n_unconverged") *val = h->st_nunconv;
+  else if (k == "gemm_launches") *val = h->st_gemm_launches;
+  else if (k == "kernel_launches") *val = h->st_kernel_launches;
+  else if (k == "panel_ni") *val = h->panel_ni;
+  else if (k == "gmres_m_used") *val = h->sw.m;
+  else if (k == "reset_counters") { *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = 0; }
+  else { h->err = "gfcc_get_stat: unknown key " + k; return GFCC_EINVAL; }
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_get_residuals(gfcc_handle h, int n, double* relres, int* iters) {
+  if (!h || n < 0 || (size_t)n > h->last_relres.size()) return GFCC_EINVAL;
+  for (int k = 0; k < n; ++k) {
+    if (relres) relres[k] = h->last_relres[k];
+    if (iters) iters[k] = h->last_iters[k];
+  }
+  return GFCC_OK;
+}
+
+extern "C" long long gfcc_get_intermediate(gfcc_handle h, const char* name, double* out) {
+  if (!h || !name) return GFCC_EINVAL;
+  const long long o = h->o, v = h->v, Q = h->Q, np_ = h->npair;
+  std::string k(name);
+  const double* src = nullptr; long long n = 0;
+  if (k == "Fme") { src = h->Fme; n = o * v; }
+  else if (k == "Fmi") { src = h->Fmi; n = o * o; }
+  else if (k == "Fae") { src = h->Fae; n = v * v; }
+  else if (k == "Wmnij") { src = h->Wp; n = np_ * np_; }
+  else if (k == "Wmbij") { src = h->WB; n = np_ * v * o; }
+  else if (k == "D") { src = h->D; n = o * o; }
+  else if (k == "Lm") { src = h->Lm; n = Q * o * v; }
+  else { h->err = "gfcc_get_intermediate: unknown name " + k; return GFCC_EINVAL; }
+  if (out) {
+    if (cudaMemcpyAsync(out, src, (size_t)n * 8, cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) { h->err = "copy failed"; return GFCC_ECUDA; }
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "sync failed"; return GFCC_ECUDA; }
+  }
+  return n;
+}
+
+// ------------------------------------------------------------------------------------------
+// gfcc_sigma_ip
+// ------------------------------------------------------------------------------------------
+static int sigma_abi(gfcc_handle h, int nrhs, const double* omega, double eta, const void* X1, const void* X2, void* S1, void* S2) {
+  const int o = h->o, v = h->v;
+  TRY(ensure_workspace(h, nrhs, true));
+  cudaStream_t st = h->stream;
+  CUDA_TRY(h, cudaMemcpyAsync(h->d_omega, omega, (size_t)nrhs * 8, cudaMemcpyHostToDevice, st));
+  dim3 blk(32, 8), grid((unsigned)((h->nvec + 31) / 32), (unsigned)((nrhs + 31) / 32));
+  k_abi_to_vec<<<grid, blk, 0, st>>>(h->vin, (const double2*)X1, (const double2*)X2, o, v, nrhs);
+  KLAUNCH(h);
+  TRY(sigma_internal(h, nrhs, h->d_omega, eta, h->vin, h->vout));
+  k_vec_to_abi<<<grid, blk, 0, st>>>((double2*)S1, (double2*)S2, h->vout, o, v, nrhs);
+  KLAUNCH(h);
+  k_zero_diag<<<nblk((long long)nrhs * o * v), 256, 0, st>>>((double2*)S2, o, v, nrhs);
+  KLAUNCH(h);
+  h->st_flops_sigma = sigma_flops(h, nrhs);
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_sigma_ip(gfcc_handle h, int nrhs, const double* omega, double eta, const void* X1, const void* X2,
+                             void* S1, void* S2) {
+  if (!h) return GFCC_EINVAL;
+  if (nrhs < 1 || !omega || !X1 || !X2 || !S1 || !S2) { h->err = "gfcc_sigma_ip: null pointer or nrhs < 1"; return GFCC_EINVAL; }
+  return sigma_abi(h, nrhs, omega, eta, X1, X2, S1, S2);
+}
+
+extern "C" int gfcc_sigma_ip_host(gfcc_handle h, int nrhs, const double* omega, double eta, const void* X1, const void* X2,
+                                  void* S1, void* S2) {
+  if (!h) return GFCC_EINVAL;
+  if (nrhs < 1 || !omega || !X1 || !X2 || !S1 || !S2) { h->err = "gfcc_sigma_ip_host: null pointer or nrhs < 1"; return GFCC_EINVAL; }
+  const long long o = h->o, v = h->v;
+  const long long n1 = (long long)nrhs * o * 2, n2 = (long long)nrhs * o * o * v * 2;
+  TRY(ensure_workspace(h, nrhs, true));
+  // stage the ABI-layout vectors in the Z and V scratch (each o*v*o*Nc doubles = exactly one X2 batch)
+  double* dX2 = h->V;      // V is written late in sigma_internal, after vin has been built
+  double* dS2 = h->XU;     // XU is dead when the result is unpacked
+  double *dX1 = nullptr, *dS1 = nullptr;
+  TRY(dev_alloc(h, &dX1, n1)); TRY(dev_alloc(h, &dS1, n1));
+  cudaStream_t st = h->stream;
+  int rc = GFCC_OK;
+  do {
+    if (cudaMemcpyAsync(dX1, X1, (size_t)n1 * 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(dX2, X2, (size_t)n2 * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) { h->err = "H2D copy failed"; rc = GFCC_ECUDA; break; }
+    rc = sigma_abi(h, nrhs, omega, eta, dX1, dX2, dS1, dS2);
+    if (rc) break;
+    if (cudaMemcpyAsync(S1, dS1, (size_t)n1 * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(S2, dS2, (size_t)n2 * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) { h->err = "D2H copy failed"; rc = GFCC_ECUDA; break; }
+    if (cudaStreamSynchronize(st) != cudaSuccess) { h->err = "sync failed"; rc = GFCC_ECUDA; }
+  } while (0);
+  cudaStreamSynchronize(st);
+  dev_free(h, dX1, n1); dev_free(h, dS1, n1);
+  return rc;
+}
+
+extern "C" int gfcc_dgemm(void* stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
+                          const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn) {
+  if (M < 0 || N < 0 || K < 0 || !A || !B || !C) return GFCC_EINVAL;
+  if ((sAm != 1 && sAk != 1) || (sBk != 1 && sBn != 1)) return GFCC_EINVAL;
+  GemmDesc d; d.M = M; d.N = N; d.K0 = K;
+  d.A = A; d.sAm = sAm; d.sAk0 = sAk; d.B = B; d.sBk0 = sBk; d.sBn = sBn;
+  if (sAk == 1 && sAm == 1) d.sAm = (K > 1) ? K : 1;   // degenerate: treat as K-contiguous row
+  d.C = C; d.sCm0 = sCm; d.sCn0 = sCn; d.alpha = alpha; d.beta = beta;
+  if (K == 0) d.K0 = 0;
+  cudaError_t e = launch_dgemm(d, (cudaStream_t)stream);
+  return e == cudaSuccess ? GFCC_OK : GFCC_ECUDA;
+}
+
+// ------------------------------------------------------------------------------------------
+// gfcc_solve_ip : batched GMRES + G assembly (gfcc_solve.cuh holds the kernels and the driver loop)
+// ------------------------------------------------------------------------------------------
+static int solve_batch(gfcc_handle h, int nrhs, const int* p_of_rhs, const double* w_of_rhs, double eta, double tol,
+                       double2* Gq_dev /* [nrhs][nq] */, const int* qlist, int nq, double* X1out, double* X2out, int rhs_offset,
+                       int nrhs_total) {
+  TRY(ensure_workspace(h, nrhs, false));
+  SolveCfg cfg;
+  cfg.o = h->o; cfg.v = h->v; cfg.nrhs = nrhs; cfg.nvec = h->nvec; cfg.npair = h->npair;
+  cfg.m = (int)h->opt_m; cfg.maxit = (int)h->opt_maxit; cfg.fixed = (int)h->opt_fixed; cfg.x0 = (int)h->opt_x0;
+  cfg.eta = eta; cfg.tol = tol;
+  cfg.t1 = h->t1; cfg.l1 = h->l1; cfg.T2p = h->T2p; cfg.L2p = h->L2p; cfg.D = h->D; cfg.fdiag = h->fdiag;
+  cfg.stream = h->stream;
+  auto apply = [&](const double* xin, double* sout) -> int { return sigma_internal(h, nrhs, h->d_omega, eta, xin, sout); };
+  std::string err;
+  double nlaunch = 0;
+  int rc = solve_run(h->sw, cfg, p_of_rhs, w_of_rhs, h->d_omega, apply, Gq_dev, qlist, nq, X1out, X2out, rhs_offset, nrhs_total,
+                     h->last_relres, h->last_iters, &h->st_iterations, &nlaunch, err);
+  h->st_kernel_launches += nlaunch;
+  if (rc == GFCC_ECUDA || rc == GFCC_ENOMEM || rc == GFCC_EINVAL) h->err = err;
+  return rc;
+}
+
+extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol,
+                               void* G, void* X1out, void* X2out) {
+  if (!h) return GFCC_EINVAL;
+  if (np < 1 || nw < 1 || !p || !omega || !G || !(tol > 0)) { h->err = "gfcc_solve_ip: null pointer, np/nw < 1 or tol <= 0"; return GFCC_EINVAL; }
+  for (int k = 0; k < np; ++k)
+    if (p[k] < 0 || p[k] >= h->N) { h->err = "gfcc_solve_ip: target orbital out of range"; return GFCC_EINVAL; }
+  const int ntot = np * nw;
+  h->last_relres.assign(ntot, 0.0);
+  h->last_iters.assign(ntot, 0);
+  h->st_iterations = 0;
+  std::vector<int> pr(ntot);
+  std::vector<double> wr(ntot);
+  for (int ip = 0; ip < np; ++ip)
+    for (int iw = 0; iw < nw; ++iw) { pr[ip * nw + iw] = p[ip]; wr[ip * nw + iw] = omega[iw]; }
+  double* Gq = nullptr;   // [ntot][np] complex
+  TRY(dev_alloc(h, &Gq, (long long)ntot * np * 2));
+  int* dq = nullptr;
+  { double* t = nullptr; TRY(dev_alloc(h, &t, np)); dq = (int*)t; }
+  int rc_final = GFCC_OK;
+  do {
+    if (cudaMemcpyAsync(dq, p, (size_t)np * sizeof(int), cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { h->err = "H2D failed"; rc_final = GFCC_ECUDA; break; }
+    const int maxb = std::max(1, (int)h->opt_max_batch);
+    // equal-sized batches so that the workspace is allocated once
+    const int nb = (ntot + maxb - 1) / maxb;
+    const int bsz = (ntot + nb - 1) / nb;
+    for (int r0 = 0; r0 < ntot; r0 += bsz) {
+      const int n = std::min(bsz, ntot - r0);
+      int rc = solve_batch(h, n, pr.data() + r0, wr.data() + r0, eta, tol, (double2*)Gq + (long long)r0 * np, dq, np,
+                           (double*)X1out, (double*)X2out, r0, ntot);
+      if (rc == GFCC_ENOCONV) rc_final = GFCC_ENOCONV;
+      else if (rc != GFCC_OK) { rc_final = rc; break; }
+    }
+    if (rc_final != GFCC_OK && rc_final != GFCC_ENOCONV) break;
+    // G[iw][ip][iq] <- Gq[(ip*nw+iw)][iq]
+    std::vector<double> hostG((size_t)ntot * np * 2), outG((size_t)ntot * np * 2);
+    if (cudaMemcpyAsync(hostG.data(), Gq, hostG.size() * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "D2H of G failed"; rc_final = GFCC_ECUDA; break; }
+    for (int ip = 0; ip < np; ++ip)
+      for (int iw = 0; iw < nw; ++iw)
+        for (int iq = 0; iq < np; ++iq)
+          for (int c = 0; c < 2; ++c)
+            outG[(((size_t)iw * np + ip) * np + iq) * 2 + c] = hostG[(((size_t)ip * nw + iw) * np + iq) * 2 + c];
+    if (cudaMemcpy(G, outG.data(), outG.size() * 8, cudaMemcpyDefault) != cudaSuccess) { h->err = "copy of G to the caller failed"; rc_final = GFCC_ECUDA; break; }
+  } while (0);
+  cudaStreamSynchronize(h->stream);
+  dev_free(h, Gq, (long long)ntot * np * 2);
+  dev_free(h, (double*)dq, np);
+  h->st_max_relres = 0; h->st_nunconv = 0;
+  for (int k = 0; k < ntot; ++k) {
+    h->st_max_relres = std::max(h->st_max_relres, h->last_relres[k]);
+    if (h->opt_fixed == 0 && !(h->last_relres[k] <= tol)) h->st_nunconv += 1;
+  }
+  h->st_flops_sigma = sigma_flops(h, h->ws_nrhs > 0 ? h->ws_nrhs : 1);
+  return rc_final;
+}
+
+extern "C" int gfcc_solve_ip(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol, void* G) {
+  return gfcc_solve_ip_x(h, np, p, nw, omega, eta, tol, G, nullptr, nullptr);
+}
