@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py -- GFCCSD-IP hot path on B200: sigma-matvec FP64 TFLOP/s and (p,omega) solves/s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+    torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...      (one rank per GPU)
+
+A STEP is one pass of the whole hot path over one batch of synthetic right-hand sides: one gfcc_solve_ip call
+in fixed-iteration mode (gmres_fixed = KFIX Arnoldi steps => KFIX+1 batched sigma applications S1-S13, the
+CGS2/Givens work G1-G5 and the G_pq assembly G6).  The one-time intermediates (gfcc_create, P1-P7, PAPER.md:173
+"pre-computed before entering the main GFCC loop") are built before the timed region and reported as create_s.
+`value` = (KFIX+1) * F_sigma / step time: sigma FP64 TFLOP/s of the WHOLE step (GMRES and G time are charged
+against it); F_sigma is the executed flop model of SURVEY.md 8(d) (real x complex counted as 2 real products,
+pair-packed o^4 term).  N > 1: the (p,omega) list is sharded over ranks (independent tasks),
+no data-path collective, weak scaling.
+
+Inputs are seeded and synthetic (gfcc_inputs) and stand in for the paper's molecular
+workloads.  The working set of every config >= 1 is far larger than the 126 MB L2.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FP64_DMMA_PEAK_TFLOPS = 36.95   # measured on this pool's B200: DMMA.8x8x4 issue-rate probe (profiles/fp64_peak_probe.md)
+KFIX = {0: 20, 1: 8, 2: 4, 3: 2, 4: 1}      # Arnoldi steps per timed step (bounded so that a default run ends in minutes)
+DEFAULT_CONFIG = 4
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kfix", type=int, default=0, help="Arnoldi steps per step (default: per config)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+
+    def __init__(self, gpu_index):
+        super().__init__(daemon=True)
+        self.gpu = gpu_index
+        self.samples, self.reasons, self.maxclk = [], set(), None
+        self.stop_flag = False
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.gpu)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip().split(",")
+                self.samples.append(float(out[0]))
+                self.maxclk = float(out[1])
+                for n, val in zip(names, out[2:]):
+                    if "Active" in val and "Not" not in val:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.maxclk, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def workload_string(cfg, c, nrhs, kfix, rank_shift):
+    return (f"config{cfg}: o={c['o']} v={c['v']} Q={c['Q']} nrhs={nrhs} ({c['np']} p x {c['nw']} omega per GPU), eta={c['eta']}, "
+            f"one gfcc_solve_ip with {kfix} fixed Arnoldi steps = {kfix + 1} batched sigma applications + CGS2/Givens + G assembly")
+
+
+# ---------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, c, nsamp, nrhs_s, threads_note=True):
+    """time the CPU oracle (as it stands) on a bounded sample of the workload; returns (seconds, description, cores)."""
+    import torch
+    import gfcc_inputs as gi
+    import oracle
+    o, v, Q = c["o"], c["v"], c["Q"]
+    dev = "cuda" if (torch.cuda.is_available() and cfg >= 2) else "cpu"
+    s = gi.make_config(cfg, dev)
+    host = {k: s[k].cpu().numpy() for k in ("fock", "T1", "T2p", "L1", "L2p", "Lchol")}
+    X1, X2 = gi.trial_vectors(o, v, nrhs_s, gi.seed_of(cfg), dev)
+    X1, X2 = X1.cpu().numpy(), X2.cpu().numpy()
+    del s
+    if dev == "cuda":
+        torch.cuda.empty_cache()
+    w = np.linspace(c["wlo"], c["whi"], nrhs_s)
+    if cfg <= 1 and False:
+        pass
+    t0 = time.time()
+    orc = oracle.Oracle(o, v, Q, host["fock"], host["T1"], host["T2p"], host["L1"], host["L2p"], host["Lchol"], oracle.MODE_ROWS)
+    t_setup = time.time() - t0
+    rng = np.random.default_rng(7)
+    trip = np.stack([rng.integers(0, o - 1, nsamp), np.full(nsamp, o - 1), rng.integers(0, v, nsamp)], axis=1)
+    t0 = time.time()
+    orc.sigma_rows(w, c["eta"], X1, X2, [o - 1], trip)
+    t_rows = time.time() - t0
+    return t_setup, t_rows, trip, oracle.threads()
+
+
+def cpu_baseline(cfg, c, nrhs, flops_sigma):
+    nsamp, nrhs_s = (4, 2) if cfg <= 2 else ((2, 1) if cfg == 3 else (1, 1))
+    t_setup, t_rows, trip, cores = oracle_sample(cfg, c, nsamp, nrhs_s)
+    npair = c["o"] * (c["o"] - 1) // 2
+    rows_total = npair * c["v"] * nrhs
+    t_full = t_rows * rows_total / (nsamp * nrhs_s)      # linear extrapolation to all rows of all RHS
+    return {"value": flops_sigma / t_full / 1e12, "unit": "TFLOP/s", "cores": cores, "kind": "oracle",
+            "sample": (f"row-sampled oracle sigma (oracle/gfcc_oracle.cpp orc_sigma_rows): {nsamp} sigma2 rows + 1 sigma1 row x {nrhs_s} "
+                       f"RHS of config {cfg} in {t_rows:.1f} s (+{t_setup:.1f} s one-time dressing), EXTRAPOLATED linearly to the "
+                       f"{rows_total} (row,RHS) outputs of one batched application"),
+            "seconds_sample": t_rows, "seconds_setup": t_setup}
+
+
+# ---------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import gfcc_inputs as gi
+    cfg = args.config
+    c = gi.CONFIGS[cfg]
+    nrhs = c["np"] * c["nw"]
+    kfix = args.kfix or KFIX[cfg]
+    o, v, Q = c["o"], c["v"], c["Q"]
+    npair = o * (o - 1) // 2
+    Nc = 2.0 * nrhs
+    ov = o * v
+    flops_sigma = (2 * Q * ov * o * Nc * 2 + 4 * Q * ov * ov + 6 * ov * ov * o * Nc + 2 * npair * npair * v * Nc
+                   + 2 * npair * v * v * Nc + 2 * npair * v * o * Nc + 2 * Q * o * v * Nc + 2 * Q * o * o * Nc + 2 * ov * o * Nc)
+    vals = []
+    last = None
+    for it in range(args.warmup + args.steps):
+        cb = cpu_baseline(cfg, c, nrhs, flops_sigma)
+        if it >= args.warmup:
+            vals.append(cb["value"])
+        last = cb
+        if it == 0 and cb["seconds_sample"] + cb["seconds_setup"] > 60:
+            # one sample already takes a minute: do not repeat it warmup+steps times
+            vals = [cb["value"]]
+            break
+    value = float(np.mean(vals))
+    npair_rows = npair * v * nrhs
+    line = {"impl": "reference", "metric": "sigma_matvec_fp64_tflops", "value": value, "unit": "TFLOP/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": (kfix + 1) * flops_sigma / (value * 1e12) * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_string(cfg, c, nrhs, kfix, 0), "l2": "working set >> 126 MB L2"},
+            "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
+            "e2e": {"value": value, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "note": f"extrapolated from sampled rows ({npair_rows} outputs per application)"}
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import gfcc_inputs as gi
+    import paper_2010_04768_b200 as g
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = args.config
+    c = gi.CONFIGS[cfg]
+    o, v, Q = c["o"], c["v"], c["Q"]
+    nrhs = c["np"] * c["nw"]
+    kfix = args.kfix or KFIX[cfg]
+
+    # ---- inputs (seeded, generated directly in HBM) and one-time intermediates ----
+    t0 = time.time()
+    s = gi.make_config(cfg, "cuda")
+    torch.cuda.synchronize()
+    t_inputs = time.time() - t0
+    t0 = time.time()
+    h = g.gfcc_create(o, v, Q, s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+    torch.cuda.synchronize()
+    create_s = time.time() - t0
+    flops_create = g.gfcc_get_stat(h, "flops_create")
+    del s["Lchol"]
+    torch.cuda.empty_cache()
+    stream = torch.cuda.Stream()
+    g.gfcc_set_stream(h, stream)
+    g.gfcc_set_option(h, "gmres_fixed", kfix)
+    g.gfcc_set_option(h, "max_batch", nrhs)
+
+    # rank r solves its own slice of the omega sweep (independent (p,omega) tasks; weak scaling)
+    wgrid = np.linspace(c["wlo"], c["whi"], c["nw"] * max(world, 1))
+    omegas = wgrid[rank * c["nw"]:(rank + 1) * c["nw"]]
+    targets = gi.targets(cfg)
+
+    def step():
+        return g.gfcc_solve_ip(h, targets, omegas, c["eta"], c["tol"])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    flops_sigma = g.gfcc_get_stat(h, "flops_sigma")
+    g.gfcc_get_stat(h, "reset_counters")
+    g.gfcc_set_option(h, "profile_gemm", 1)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(args.steps):
+            G = step()
+        e1.record(stream)
+    barrier()
+    sampler.stop_flag = True
+    ms_total = e0.elapsed_time(e1)
+    launches = g.gfcc_get_stat(h, "kernel_launches")
+    gemm_ms = g.gfcc_get_stat(h, "gemm_time_ms")
+    gemm_flops = g.gfcc_get_stat(h, "gemm_flops_timed")
+    gemm_n = g.gfcc_get_stat(h, "gemm_launches_timed")
+    napply = g.gfcc_get_stat(h, "sigma_applications")
+    g.gfcc_set_option(h, "profile_gemm", 0)
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    apps_per_step = napply / args.steps
+    value = world * apps_per_step * flops_sigma / (ms_step * 1e-3) / 1e12
+    solves_per_s = world * nrhs / (ms_step * 1e-3)
+
+    line = {
+        "metric": "sigma_matvec_fp64_tflops", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_string(cfg, c, nrhs, kfix, rank), "l2": "inputs and working set >> 126 MB L2 (no flush needed)",
+                   "flop_model": "executed Cholesky-route model, SURVEY.md 8(d): real x complex = 2 real products, pair-packed o^4 term",
+                   "flops_per_sigma_application": flops_sigma, "sigma_applications_per_step": apps_per_step,
+                   "gmres_m_used": g.gfcc_get_stat(h, "gmres_m_used"), "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
+        "solves_per_s": solves_per_s, "solves_note": f"(p,omega) right-hand sides advanced by {kfix} GMRES steps per second x nrhs",
+        "pct_fp64_peak_measured": 100.0 * value / world / FP64_DMMA_PEAK_TFLOPS,
+        "create_s": create_s, "create_tflops": flops_create / create_s / 1e12, "inputs_s": t_inputs,
+        "device_bytes": g.gfcc_get_stat(h, "bytes_device"), "gpu_launches": int(launches),
+    }
+    line["clocks"] = sampler.summary()
+
+    # ---- roofline of the dominant kernel (dgemm_dmma_kernel): CUDA events around every launch, on the launching stream ----
+    mp = measured_peaks()
+    achieved = gemm_flops / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+    line["roofline"] = {
+        "kernel": "gfcc::dgemm_dmma_kernel (all GEMM-engine launches of the timed region)",
+        "bound": "tensor", "achieved": achieved, "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_DMMA_PEAK_TFLOPS,
+        "peak_source": "measured FP64 DMMA.8x8x4 issue-rate ceiling on this pool's B200 (profiles/fp64_peak_probe.md); "
+                       "MEASURED_PEAKS.json has no FP64 entry",
+        "peak_alt_bf16_ratio": (mp["bf16_tflops_sustained"] * 40.0 / 2250.0) if mp else None,
+        "peak_alt_note": "sustained bf16 peak of MEASURED_PEAKS.json x nominal FP64:bf16 ratio 40/2250 (fallback rule; lower than the "
+                         "directly measured DMMA ceiling, so the stricter denominator is used for frac)",
+        "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1), "share_of_step": gemm_ms / ms_total if ms_total > 0 else None,
+        "algorithmic_flops": gemm_flops, "traffic": None,
+        "traffic_note": "DRAM bytes per launch are in profiles/ (ncu --set full of the same kernel): <3% of DRAM peak, L2 hit 82%",
+    }
+
+    # ---- end to end through the C ABI with HOST buffers: one batched sigma application, copies inside the call ----
+    if not args.no_e2e and rank == 0:
+        try:
+            X1, X2 = gi.trial_vectors(o, v, nrhs, gi.seed_of(cfg), "cuda")
+            X1h = torch.empty(X1.shape, dtype=X1.dtype, pin_memory=True).copy_(X1)
+            X2h = torch.empty(X2.shape, dtype=X2.dtype, pin_memory=True).copy_(X2)
+            del X1, X2
+            torch.cuda.empty_cache()
+            wr = np.repeat(omegas, c["np"])[:nrhs] if len(omegas) * c["np"] >= nrhs else np.resize(omegas, nrhs)
+            g.gfcc_sigma_ip_host(h, wr, c["eta"], X1h.numpy(), X2h.numpy())   # warm-up
+            nrep = 2 if cfg >= 3 else 3
+            t0 = time.perf_counter()
+            for _ in range(nrep):
+                S1h, S2h = g.gfcc_sigma_ip_host(h, wr, c["eta"], X1h.numpy(), X2h.numpy())
+            dt = (time.perf_counter() - t0) / nrep
+            nb = X1h.numel() * 16 + X2h.numel() * 16
+            line["e2e"] = {"value": flops_sigma / dt / 1e12, "unit": "TFLOP/s", "h2d_bytes_per_step": int(nb + 8 * nrhs),
+                           "d2h_bytes_per_step": int(nb), "ms_per_step": dt * 1e3,
+                           "what": "gfcc_sigma_ip_host: X1,X2 from pinned host memory, S1,S2 back to host, copies inside the timed call"}
+        except Exception as ex:   # noqa: BLE001
+            line["e2e"] = {"value": None, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": str(ex)[:200]}
+    g.gfcc_destroy(h)
+    del s
+    torch.cuda.empty_cache()
+
+    # ---- CPU baseline: the oracle on the host cores, bounded sample (rank 0, N = 1 only) ----
+    if world == 1 and not args.no_cpu_baseline:
+        try:
+            cb = cpu_baseline(cfg, c, nrhs, flops_sigma)
+            cb.pop("seconds_sample", None)
+            cb.pop("seconds_setup", None)
+            line["cpu_baseline"] = cb
+        except Exception as ex:   # noqa: BLE001
+            line["cpu_baseline"] = {"value": None, "unit": "TFLOP/s", "cores": None, "kind": "oracle", "sample": f"failed: {str(ex)[:200]}"}
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

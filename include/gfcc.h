@@ -91,7 +91,9 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *   "gmres_fixed"  if > 0: run exactly this many Arnoldi steps in ONE cycle, no stop test (timing mode)
  *   "x0"           0: zero initial guess, 1: zeroth-order guess b/(omega - i eta + d) (default 1)
  *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3e9)
- *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256) */
+ *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256)
+ *   "profile_gemm" 1: bracket every GEMM-engine launch with CUDA events on the handle's stream (statistics
+ *                  "gemm_time_ms", "gemm_flops_timed", "gemm_launches_timed"); 0: off (default) */
 int gfcc_set_option(gfcc_handle h, const char* key, double val);
 
 /* Statistics of the last call (double-valued): "iterations" (Arnoldi steps of the last solve),

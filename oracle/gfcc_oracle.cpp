@@ -344,17 +344,24 @@ void build_dressed(Ctx& c) {
         c.Lvv[((i64)a * v + e) * Q + k] = acc;
       }
   // Lvo[a,i] = L_ai - sum_m t[m,a] L_mi + sum_e t[i,e] L_ae - sum_me t[m,a] t[i,e] L_me
+  //          = L_ai - sum_m t[m,a] L_mi + sum_e t[i,e] ( L_ae - sum_m t[m,a] L_me )      [ (A^T L) B, SURVEY.md 8a P1 ]
+  //          = L_ai - sum_m t[m,a] L_mi + sum_e t[i,e] Lvv[a,e]        with the dressed Lvv computed just above
+  // (the bracketed sum is taken once per (a,e) instead of once per (a,i,e): same terms, O(Q v o (o+v)) work)
 #pragma omp parallel for collapse(2)
   for (int a = 0; a < v; ++a)
-    for (int i = 0; i < o; ++i)
-      for (int k = 0; k < Q; ++k) {
-        double acc = Lg(k, o + a, i);
-        for (int m = 0; m < o; ++m) acc -= T1(m, a) * Lg(k, m, i);
-        for (int e = 0; e < v; ++e) acc += T1(i, e) * Lg(k, o + a, o + e);
-        for (int m = 0; m < o; ++m)
-          for (int e = 0; e < v; ++e) acc -= T1(m, a) * T1(i, e) * Lg(k, m, o + e);
-        c.Lvo[((i64)a * o + i) * Q + k] = acc;
+    for (int i = 0; i < o; ++i) {
+      double* dst = &c.Lvo[((i64)a * o + i) * Q];
+      for (int k = 0; k < Q; ++k) dst[k] = Lg(k, o + a, i);
+      for (int m = 0; m < o; ++m) {
+        const double t = T1(m, a);
+        for (int k = 0; k < Q; ++k) dst[k] -= t * Lg(k, m, i);
       }
+      for (int e = 0; e < v; ++e) {
+        const double t = T1(i, e);
+        const double* lv = &c.Lvv[((i64)a * v + e) * Q];
+        for (int k = 0; k < Q; ++k) dst[k] += t * lv[k];
+      }
+    }
   // dressed Fock: ft = A^T ( f + J - K ) B,  (f+J-K)_pq = f_pq + sum_kc t[k,c] <pk||qc>
   std::vector<double> s(Q, 0.0), g((size_t)N * N, 0.0), U((size_t)Q * N * o, 0.0);
   for (int k = 0; k < Q; ++k) {

@@ -7,9 +7,10 @@
 // sm_100a is DMMA: mma.sync.aligned.m8n8k4.f64 (SASS DMMA.8x8x4; the m16n8k{4,8,16} PTX shapes are
 // split into 8x8x4 by ptxas on this target).  Measured issue-rate ceiling on B200: 36.95 TFLOP/s.
 //
-// Kernel: CTA tile BM x 128 x 16 with BM = 16*WMF (WMF = m8 fragments per warp, chosen per problem
-// to avoid ragged-M waste), 8 warps as 2(M) x 4(N), warp tile (8*WMF) x 32, accumulators in registers,
-// 4-stage cp.async (LDGSTS) shared-memory pipeline with padded, bank-conflict-free tiles.
+// Kernel: CTA tile BM x 128 x 16 with BM = WGM*8*WMF (WMF = m8 fragments per warp, chosen per problem
+// to avoid ragged-M waste), WGM x 4 warps (default WGM = 2: 8 warps, warp tile up to 64 x 32), accumulators in
+// registers, fragments double-buffered in registers across k4 steps and across tiles, 4-stage cp.async
+// (LDGSTS) shared-memory pipeline with padded, bank-conflict-free tiles.
 //
 // Operand addressing (element strides, FP64):
 //   A(m, k1, k0) = A + offA(k1) + m*sAm + k0*sAk0      B(k1, k0, n) = B + offB(k1) + k0*sBk0 + n*sBn
@@ -22,6 +23,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 namespace gfcc {
 
@@ -40,11 +42,11 @@ struct GemmParams {
 constexpr int GEMM_BN = 128;
 constexpr int GEMM_BK = 16;
 constexpr int GEMM_STAGES = 4;
-constexpr int GEMM_THREADS = 256;
 constexpr int GEMM_PAD = 4;   // doubles; makes every fragment load bank-conflict free (ld % 16 == 4)
 
-template <int WMF> struct GemmTile {
-  static constexpr int BM = 16 * WMF;
+template <int WGM, int WMF> struct GemmTile {
+  static constexpr int THREADS = WGM * 4 * 32;
+  static constexpr int BM = WGM * 8 * WMF;
   static constexpr int LDK = GEMM_BK + GEMM_PAD;             // K-contiguous tiles: [rows][LDK]
   static constexpr int LDA_M = BM + GEMM_PAD;                // M-contiguous A tile: [BK][LDA_M]
   static constexpr int LDB_N = GEMM_BN + GEMM_PAD;           // N-contiguous B tile: [BK][LDB_N]
@@ -72,19 +74,24 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 
 // copy one 2-double chunk (contiguous in global memory) into shared memory with zero fill.
 // nvalid in {0,1,2}: number of in-range elements of the chunk.
-__device__ __forceinline__ void load_chunk(double* sdst, const double* gsrc, int nvalid, int vec) {
+// `safe` is any valid address of the operand (used when the chunk is entirely out of range: src-size 0).
+__device__ __forceinline__ void load_chunk(double* sdst, const double* gsrc, int nvalid, int vec, const double* safe) {
   if (vec) {
-    cp_async16(sdst, nvalid > 0 ? gsrc : nullptr, nvalid > 0 ? nvalid * 8 : 0);
+    cp_async16(sdst, nvalid > 0 ? gsrc : safe, nvalid > 0 ? nvalid * 8 : 0);
   } else {
-    cp_async8(sdst, nvalid > 0 ? gsrc : nullptr, nvalid > 0 ? 8 : 0);
-    cp_async8(sdst + 1, nvalid > 1 ? gsrc + 1 : nullptr, nvalid > 1 ? 8 : 0);
+    cp_async8(sdst, nvalid > 0 ? gsrc : safe, nvalid > 0 ? 8 : 0);
+    cp_async8(sdst + 1, nvalid > 1 ? gsrc + 1 : safe, nvalid > 1 ? 8 : 0);
   }
 }
 
-template <int WMF, bool A_KC, bool B_NC>
-__global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmParams p) {
-  using T = GemmTile<WMF>;
-  constexpr int BM = T::BM, BN = GEMM_BN, BK = GEMM_BK;
+__device__ __forceinline__ double flip_sign(double x, unsigned mask) {
+  return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));   // integer pipe, not the FP64 pipe
+}
+
+template <int WGM, int WMF, bool A_KC, bool B_NC, bool HAS_SIGN>
+__global__ void __launch_bounds__(WGM * 128, 1) dgemm_dmma_kernel(const GemmParams p) {
+  using T = GemmTile<WGM, WMF>;
+  constexpr int BM = T::BM, BN = GEMM_BN, BK = GEMM_BK, GEMM_THREADS = T::THREADS;
   extern __shared__ __align__(16) double smem[];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -109,16 +116,17 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmP
   const double* __restrict__ Bb = p.B + (long long)z * p.bsB;
   const long long* tabA = p.tabA ? p.tabA + (long long)z * p.tab_batch_stride : nullptr;
   const long long* tabB = p.tabB ? p.tabB + (long long)z * p.tab_batch_stride : nullptr;
-  const double* sgn = p.sgn ? p.sgn + (long long)z * p.tab_batch_stride : nullptr;
+  const double* sgn = HAS_SIGN ? p.sgn + (long long)z * p.tab_batch_stride : nullptr;
 
   const int KT0 = (p.K0 + BK - 1) / BK;
   int nblocks = 0;   // number of non-skipped k1 blocks
-  for (int k1 = 0; k1 < p.K1; ++k1) nblocks += (sgn == nullptr || sgn[k1] != 0.0) ? 1 : 0;
+  if (HAS_SIGN) { for (int k1 = 0; k1 < p.K1; ++k1) nblocks += (sgn[k1] != 0.0) ? 1 : 0; }
+  else nblocks = p.K1;
   const int total = nblocks * KT0;
 
   // ---- loader state: (k1, kt) of the next tile to fetch
   int ld_k1 = 0, ld_kt = 0, ld_count = 0;
-  auto skip_zero = [&](int& k1) { while (sgn != nullptr && k1 < p.K1 && sgn[k1] == 0.0) ++k1; };
+  auto skip_zero = [&](int& k1) { if (HAS_SIGN) { while (k1 < p.K1 && sgn[k1] == 0.0) ++k1; } };
   skip_zero(ld_k1);
 
   auto issue_load = [&](int stage) {
@@ -134,7 +142,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmP
         const int row = c / CPR, kc = (c % CPR) * 2;
         const int gm = m0 + row, gk = k0 + kc;
         int nv = (gm < p.M) ? min(2, max(0, p.K0 - gk)) : 0;
-        load_chunk(As + row * T::LDK + kc, Ab + offA + (long long)gm * p.sAm + gk, nv, p.vecA);
+        load_chunk(As + row * T::LDK + kc, Ab + offA + (long long)gm * p.sAm + gk, nv, p.vecA, p.A);
       }
     } else {      // As[BK][LDA_M], chunks along m
       constexpr int CPR = BM / 2;
@@ -143,7 +151,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmP
         const int kr = c / CPR, mc = (c % CPR) * 2;
         const int gm = m0 + mc, gk = k0 + kr;
         int nv = (gk < p.K0) ? min(2, max(0, p.M - gm)) : 0;
-        load_chunk(As + kr * T::LDA_M + mc, Ab + offA + (long long)gk * p.sAk0 + gm, nv, p.vecA);
+        load_chunk(As + kr * T::LDA_M + mc, Ab + offA + (long long)gk * p.sAk0 + gm, nv, p.vecA, p.A);
       }
     }
     if (B_NC) {   // Bs[BK][LDB_N], chunks along n
@@ -153,7 +161,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmP
         const int kr = c / CPR, nc = (c % CPR) * 2;
         const int gn = n0 + nc, gk = k0 + kr;
         int nv = (gk < p.K0) ? min(2, max(0, p.N - gn)) : 0;
-        load_chunk(Bs + kr * T::LDB_N + nc, Bb + offB + (long long)gk * p.sBk0 + gn, nv, p.vecB);
+        load_chunk(Bs + kr * T::LDB_N + nc, Bb + offB + (long long)gk * p.sBk0 + gn, nv, p.vecB, p.B);
       }
     } else {      // Bs[BN][LDK], chunks along k
       constexpr int CPR = BK / 2;
@@ -162,7 +170,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmP
         const int col = c / CPR, kc = (c % CPR) * 2;
         const int gn = n0 + col, gk = k0 + kc;
         int nv = (gn < p.N) ? min(2, max(0, p.K0 - gk)) : 0;
-        load_chunk(Bs + col * T::LDK + kc, Bb + offB + (long long)gn * p.sBn + gk, nv, p.vecB);
+        load_chunk(Bs + col * T::LDK + kc, Bb + offB + (long long)gn * p.sBn + gk, nv, p.vecB, p.B);
       }
     }
     // advance loader
@@ -191,34 +199,54 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) dgemm_dmma_kernel(const GemmP
   const int bcol = wn * 32 + (lane >> 2);          // + 8 g
   const int kl = lane & 3;
 
+  // register double buffer of fragments: the fragments of k4-step kk+1 (or of step 0 of the NEXT tile) are
+  // loaded while the DMMAs of step kk issue, so that neither LDS latency nor the per-tile barrier leaves the
+  // DMMA pipe idle.  Requires tiles `it` and `it+1` to be resident at the top of iteration `it`.
+  double fa[2][WMF], fb[2][4];
+  auto load_frags = [&](int buf, int stage, int kk, unsigned smask) {
+    const double* As = smem + (size_t)stage * T::STAGE_ELEMS;
+    const double* Bs = As + T::A_ELEMS;
+    const int k = kk * 4 + kl;
+#pragma unroll
+    for (int f = 0; f < WMF; ++f)
+      fa[buf][f] = A_KC ? As[(arow + 8 * f) * T::LDK + k] : As[k * T::LDA_M + arow + 8 * f];
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+      const double bv = B_NC ? Bs[k * T::LDB_N + bcol + 8 * g] : Bs[(bcol + 8 * g) * T::LDK + k];
+      fb[buf][g] = HAS_SIGN ? flip_sign(bv, smask) : bv;
+    }
+  };
+  auto mask_of = [&](int k1) -> unsigned { return (HAS_SIGN && k1 < p.K1 && sgn[k1] < 0.0) ? 0x80000000u : 0u; };
+
+  cp_async_wait<GEMM_STAGES - 3>();
+  __syncthreads();
+  if (total > 0) load_frags(0, 0, 0, mask_of(c_k1));
+
   for (int it = 0; it < total; ++it) {
-    cp_async_wait<GEMM_STAGES - 2>();
-    __syncthreads();
+    if (it > 0) {
+      cp_async_wait<GEMM_STAGES - 3>();   // tiles it and it+1 have landed
+      __syncthreads();                    // ... for every thread; and everyone is done with tile it-1
+    }
     {   // prefetch tile it + STAGES - 1 into the stage consumed in iteration it-1
       if (ld_count < total) issue_load((it + GEMM_STAGES - 1) % GEMM_STAGES);
       cp_async_commit();
     }
-    const double* As = smem + (size_t)(it % GEMM_STAGES) * T::STAGE_ELEMS;
-    const double* Bs = As + T::A_ELEMS;
-    const bool neg = (sgn != nullptr) && (sgn[c_k1] < 0.0);
+    // (k1, kt) of the next tile, for the sign of the prefetched fragments
+    int n_k1 = c_k1, n_kt = c_kt + 1;
+    if (n_kt == KT0) { n_kt = 0; ++n_k1; skip_zero(n_k1); }
+    const unsigned cur_mask = mask_of(c_k1), nxt_mask = mask_of(n_k1);
+    const int stage = it % GEMM_STAGES;
 #pragma unroll
     for (int kk = 0; kk < BK / 4; ++kk) {
-      double a[WMF], b[4];
-      const int k = kk * 4 + kl;
-#pragma unroll
-      for (int f = 0; f < WMF; ++f)
-        a[f] = A_KC ? As[(arow + 8 * f) * T::LDK + k] : As[k * T::LDA_M + arow + 8 * f];
-#pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        double bv = B_NC ? Bs[k * T::LDB_N + bcol + 8 * g] : Bs[(bcol + 8 * g) * T::LDK + k];
-        b[g] = neg ? -bv : bv;
-      }
+      const int cur = kk & 1, nxt = cur ^ 1;
+      if (kk + 1 < BK / 4) load_frags(nxt, stage, kk + 1, cur_mask);
+      else if (it + 1 < total) load_frags(nxt, (it + 1) % GEMM_STAGES, 0, nxt_mask);
 #pragma unroll
       for (int f = 0; f < WMF; ++f)
 #pragma unroll
-        for (int g = 0; g < 4; ++g) dmma884(acc[f][g][0], acc[f][g][1], a[f], b[g]);
+        for (int g = 0; g < 4; ++g) dmma884(acc[f][g][0], acc[f][g][1], fa[cur][f], fb[cur][g]);
     }
-    if (++c_kt == KT0) { c_kt = 0; ++c_k1; skip_zero(c_k1); }
+    c_k1 = n_k1; c_kt = n_kt;
   }
   cp_async_wait<0>();
 
@@ -280,23 +308,32 @@ struct GemmDesc {
   bool tabs_even = true;   // caller's promise that every table offset is even (16-byte alignment)
 };
 
-// choose the m8-fragment count per warp (BM = 16*WMF) that wastes the fewest padded rows
-inline int pick_wmf(int M) {
-  int best = 8; long long bestcost = -1;
-  for (int w = 8; w >= 4; --w) {
-    const int bm = 16 * w;
+// warp-grid rows: 2 (8 warps per CTA, WMF in 4..8; measured 31.0 TFLOP/s on 8192^3) by default;
+// GFCC_GEMM_WGM=4 selects the 16-warp variant (WMF 2..4; measured 28.9 TFLOP/s) for experiments.
+inline int gemm_wgm() {
+  static int w = -1;
+  if (w < 0) { const char* e = getenv("GFCC_GEMM_WGM"); w = (e && e[0] == '4') ? 4 : 2; }
+  return w;
+}
+// choose the m8-fragment count per warp (BM = WGM*8*WMF) that wastes the fewest padded rows
+inline int pick_wmf(int M, int wgm = gemm_wgm()) {
+  const int hi = (wgm == 4) ? 4 : 8, lo = (wgm == 4) ? 2 : 4;
+  int best = hi; long long bestcost = -1;
+  for (int w = hi; w >= lo; --w) {
+    const int bm = wgm * 8 * w;
     const long long tiles = (M + bm - 1) / bm;
     // cost ~ padded rows, with a mild penalty for small tiles (lower operand reuse)
-    const long long cost = tiles * bm * 100 + (8 - w) * (long long)M;
+    const long long cost = tiles * bm * 100 + (hi - w) * 2LL * (long long)M;
     if (bestcost < 0 || cost < bestcost) { bestcost = cost; best = w; }
   }
   return best;
 }
+inline int gemm_bm(int M) { return gemm_wgm() * 8 * pick_wmf(M); }
 
-template <int WMF, bool A_KC, bool B_NC>
+template <int WGM, int WMF, bool A_KC, bool B_NC, bool HAS_SIGN>
 inline cudaError_t launch_dgemm_t(const GemmParams& p, cudaStream_t st) {
-  using T = GemmTile<WMF>;
-  auto kern = dgemm_dmma_kernel<WMF, A_KC, B_NC>;
+  using T = GemmTile<WGM, WMF>;
+  auto kern = dgemm_dmma_kernel<WGM, WMF, A_KC, B_NC, HAS_SIGN>;
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES);
@@ -304,19 +341,30 @@ inline cudaError_t launch_dgemm_t(const GemmParams& p, cudaStream_t st) {
     configured = true;
   }
   dim3 grid((unsigned)(p.tiles_m * p.tiles_n), 1, (unsigned)p.batch);
-  kern<<<grid, GEMM_THREADS, T::SMEM_BYTES, st>>>(p);
+  kern<<<grid, T::THREADS, T::SMEM_BYTES, st>>>(p);
   return cudaGetLastError();
 }
 
-template <bool A_KC, bool B_NC>
-inline cudaError_t launch_dgemm_w(int wmf, const GemmParams& p, cudaStream_t st) {
-  switch (wmf) {
-    case 8: return launch_dgemm_t<8, A_KC, B_NC>(p, st);
-    case 7: return launch_dgemm_t<7, A_KC, B_NC>(p, st);
-    case 6: return launch_dgemm_t<6, A_KC, B_NC>(p, st);
-    case 5: return launch_dgemm_t<5, A_KC, B_NC>(p, st);
-    default: return launch_dgemm_t<4, A_KC, B_NC>(p, st);
+template <bool A_KC, bool B_NC, bool HAS_SIGN>
+inline cudaError_t launch_dgemm_w(int wgm, int wmf, const GemmParams& p, cudaStream_t st) {
+  if (wgm == 4) {
+    switch (wmf) {
+      case 4: return launch_dgemm_t<4, 4, A_KC, B_NC, HAS_SIGN>(p, st);
+      case 3: return launch_dgemm_t<4, 3, A_KC, B_NC, HAS_SIGN>(p, st);
+      default: return launch_dgemm_t<4, 2, A_KC, B_NC, HAS_SIGN>(p, st);
+    }
   }
+  switch (wmf) {
+    case 8: return launch_dgemm_t<2, 8, A_KC, B_NC, HAS_SIGN>(p, st);
+    case 7: return launch_dgemm_t<2, 7, A_KC, B_NC, HAS_SIGN>(p, st);
+    case 6: return launch_dgemm_t<2, 6, A_KC, B_NC, HAS_SIGN>(p, st);
+    case 5: return launch_dgemm_t<2, 5, A_KC, B_NC, HAS_SIGN>(p, st);
+    default: return launch_dgemm_t<2, 4, A_KC, B_NC, HAS_SIGN>(p, st);
+  }
+}
+template <bool A_KC, bool B_NC>
+inline cudaError_t launch_dgemm_s(bool sign, int wgm, int wmf, const GemmParams& p, cudaStream_t st) {
+  return sign ? launch_dgemm_w<A_KC, B_NC, true>(wgm, wmf, p, st) : launch_dgemm_w<A_KC, B_NC, false>(wgm, wmf, p, st);
 }
 
 inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
@@ -334,8 +382,9 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   p.sCn0 = d.sCn0; p.sCn1 = d.sCn1; p.Nd = d.Nd > 0 ? d.Nd : (d.N > 0 ? d.N : 1);
   p.alpha = d.alpha; p.beta = d.beta;
   p.batch = d.batch; p.bsA = d.bsA; p.bsB = d.bsB; p.bsC = d.bsC; p.tab_batch_stride = d.tab_batch_stride;
-  const int wmf = pick_wmf(d.M);
-  const int bm = 16 * wmf;
+  const int wgm = gemm_wgm();
+  const int wmf = pick_wmf(d.M, wgm);
+  const int bm = wgm * 8 * wmf;
   p.tiles_m = (d.M + bm - 1) / bm;
   p.tiles_n = (d.N + GEMM_BN - 1) / GEMM_BN;
   p.group_m = 8;
@@ -344,8 +393,9 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   // 16-byte cp.async needs: aligned base, even strides along every non-contiguous direction, even offsets
   p.vecA = al16(d.A) && even(a_kc ? d.sAm : d.sAk0) && even(d.bsA) && (d.tabA ? d.tabs_even : even(d.sAk1));
   p.vecB = al16(d.B) && even(b_nc ? d.sBk0 : d.sBn) && even(d.bsB) && (d.tabB ? d.tabs_even : even(d.sBk1));
-  if (a_kc) return b_nc ? launch_dgemm_w<true, true>(wmf, p, st) : launch_dgemm_w<true, false>(wmf, p, st);
-  return b_nc ? launch_dgemm_w<false, true>(wmf, p, st) : launch_dgemm_w<false, false>(wmf, p, st);
+  const bool sign = d.sgn != nullptr;
+  if (a_kc) return b_nc ? launch_dgemm_s<true, true>(sign, wgm, wmf, p, st) : launch_dgemm_s<true, false>(sign, wgm, wmf, p, st);
+  return b_nc ? launch_dgemm_s<false, true>(sign, wgm, wmf, p, st) : launch_dgemm_s<false, false>(sign, wgm, wmf, p, st);
 }
 
 }  // namespace gfcc

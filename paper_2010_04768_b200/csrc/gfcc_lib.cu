@@ -55,6 +55,11 @@ struct gfcc_ctx {
   std::vector<double> last_relres;
   std::vector<int> last_iters;
   SolveWs sw;
+  // ---- optional per-launch timing of the GEMM engine (CUDA events on the handle's stream; bench.py roofline) ----
+  bool prof = false;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  std::vector<double> ev_flops;   // flops of the launch bracketed by events (2k, 2k+1)
 };
 
 #define CUDA_TRY(h, expr)                                                                      \
@@ -95,7 +100,17 @@ static void dev_free(gfcc_ctx* h, double* p, long long elems) {
 }
 
 static int gemm(gfcc_ctx* h, const GemmDesc& d) {
+  const bool timed = h->prof && d.M > 0 && d.N > 0 && d.K0 > 0;
+  if (timed) {
+    while (h->ev_pool.size() < h->ev_used + 2) { cudaEvent_t e; CUDA_TRY(h, cudaEventCreate(&e)); h->ev_pool.push_back(e); }
+    CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used], h->stream));
+  }
   CUDA_TRY(h, launch_dgemm(d, h->stream));
+  if (timed) {
+    CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used + 1], h->stream));
+    h->ev_used += 2;
+    h->ev_flops.push_back(2.0 * d.M * (double)d.N * (double)d.K1 * d.K0 * d.batch);
+  }
   h->st_gemm_launches += 1;
   h->st_kernel_launches += 1;
   h->st_flops_exec += 2.0 * d.M * (double)d.N * (double)d.K1 * d.K0 * d.batch;
@@ -166,7 +181,7 @@ static int choose_panel(int o, int v, long long ncols, double budget_bytes) {
   const int tiles_n = (int)((ncols + GEMM_BN - 1) / GEMM_BN);
   for (int n = nmax; n >= std::max(1, nmax / 2); --n) {
     const int rows = n * v;
-    const int bm = 16 * pick_wmf(rows);
+    const int bm = gemm_bm(rows);
     const long long tiles = (long long)((rows + bm - 1) / bm) * tiles_n;
     const long long waves = (tiles + 147) / 148;
     const double eff = (double)rows * ncols / ((double)waves * 148 * bm * GEMM_BN);
@@ -673,6 +688,7 @@ extern "C" int gfcc_destroy(gfcc_handle h) {
   cudaStreamSynchronize(h->stream);
   solve_free(h->sw);
   for (void* p : h->allocs) cudaFree(p);
+  for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   delete h;
   return GFCC_OK;
 }
@@ -694,6 +710,7 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "x0" && (val == 0 || val == 1)) h->opt_x0 = val;
   else if (k == "panel_bytes" && val > 0) { h->opt_panel_bytes = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
+  else if (k == "profile_gemm") { h->prof = (val != 0); h->ev_used = 0; h->ev_flops.clear(); }
   else { h->err = "gfcc_set_option: unknown key or invalid value: " + k; return GFCC_EINVAL; }
   return GFCC_OK;
 }
@@ -713,7 +730,16 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
   else if (k == "kernel_launches") *val = h->st_kernel_launches;
   else if (k == "panel_ni") *val = h->panel_ni;
   else if (k == "gmres_m_used") *val = h->sw.m;
-  else if (k == "reset_counters") { *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = 0; }
+  else if (k == "gemm_time_ms" || k == "gemm_flops_timed" || k == "gemm_launches_timed" || k == "gemm_time_max_ms") {
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "sync failed"; return GFCC_ECUDA; }
+    double ms = 0, fl = 0, mx = 0;
+    for (size_t q = 0; q < h->ev_flops.size(); ++q) {
+      float t = 0;
+      if (cudaEventElapsedTime(&t, h->ev_pool[2 * q], h->ev_pool[2 * q + 1]) == cudaSuccess) { ms += t; fl += h->ev_flops[q]; mx = std::max(mx, (double)t); }
+    }
+    *val = (k == "gemm_time_ms") ? ms : (k == "gemm_flops_timed") ? fl : (k == "gemm_time_max_ms") ? mx : (double)h->ev_flops.size();
+  }
+  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = 0; }
   else { h->err = "gfcc_get_stat: unknown key " + k; return GFCC_EINVAL; }
   return GFCC_OK;
 }
