@@ -183,6 +183,7 @@ def main():
     import torch
     import gfcc_inputs as gi
     import paper_2010_04768_b200 as g
+    from paper_2010_04768_b200 import sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -219,8 +220,7 @@ def main():
     g.gfcc_set_option(h, "max_batch", nrhs)
 
     # rank r solves its own slice of the omega sweep (independent (p,omega) tasks; weak scaling)
-    wgrid = np.linspace(c["wlo"], c["whi"], c["nw"] * max(world, 1))
-    omegas = wgrid[rank * c["nw"]:(rank + 1) * c["nw"]]
+    omegas = sharding.weak_scaling_grid(c["wlo"], c["whi"], c["nw"], max(world, 1), rank)
     targets = gi.targets(cfg)
 
     def step():
@@ -255,10 +255,7 @@ def main():
     gemm_n = g.gfcc_get_stat(h, "gemm_launches_timed")
     napply = g.gfcc_get_stat(h, "sigma_applications")
     g.gfcc_set_option(h, "profile_gemm", 0)
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = sharding.max_over_ranks(ms_total, world, dist, "cuda")
     ms_step = ms_total / args.steps
     apps_per_step = napply / args.steps
     value = world * apps_per_step * flops_sigma / (ms_step * 1e-3) / 1e12

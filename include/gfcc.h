@@ -120,6 +120,13 @@ int gfcc_destroy(gfcc_handle h);
 int gfcc_dgemm(void* cuda_stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
                const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn);
 
+/* Roofline denominator of the sigma contractions: measured issue-rate ceiling of the FP64 tensor-pipe instruction
+ * the GEMM engine is built on (mma.sync m8n8k4 f64 = SASS DMMA), register-only loop on every SM, CUDA events on
+ * `cuda_stream`.  iters: DMMAs per accumulator chain (>= 1; 20000 gives a ~30 ms launch); reps: timed launches
+ * (best is returned).  *tflops [host] receives TFLOP/s.  The sigma path of BASELINE.json north_star is a dense FP64
+ * contraction, MEASURED_PEAKS.json has no FP64 entry, hence this probe.                 */
+int gfcc_probe_fp64_peak(void* cuda_stream, int iters, int reps, double* tflops);
+
 #ifdef __cplusplus
 }
 #endif

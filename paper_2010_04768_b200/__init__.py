@@ -23,7 +23,7 @@ GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 
 EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_intermediate", "gfcc_last_error",
-           "gfcc_destroy", "gfcc_dgemm"]
+           "gfcc_destroy", "gfcc_dgemm", "gfcc_probe_fp64_peak"]
 
 
 class GfccError(RuntimeError):
@@ -61,6 +61,7 @@ def lib():
     L.gfcc_last_error.restype = ctypes.c_char_p
     L.gfcc_destroy.argtypes = [vp]
     L.gfcc_dgemm.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll]
+    L.gfcc_probe_fp64_peak.argtypes = [vp, ci, ci, dp]
     for name in EXPORTS:
         if name not in ("gfcc_get_intermediate", "gfcc_last_error"):
             getattr(L, name).restype = ci
@@ -233,3 +234,14 @@ def gfcc_dgemm(A, B, C=None, alpha=1.0, beta=0.0, stream=0):
     if rc != GFCC_OK:
         raise GfccError(rc, "gfcc_dgemm failed")
     return C
+
+
+def gfcc_probe_fp64_peak(iters=20000, reps=5, stream=0):
+    """Measured FP64 DMMA issue-rate ceiling of this GPU in TFLOP/s (roofline denominator of the sigma GEMMs)."""
+    _torch()
+    out = ctypes.c_double()
+    raw = getattr(stream, "cuda_stream", stream)
+    rc = lib().gfcc_probe_fp64_peak(ctypes.c_void_p(raw), int(iters), int(reps), ctypes.byref(out))
+    if rc != GFCC_OK:
+        raise GfccError(rc, "gfcc_probe_fp64_peak failed")
+    return out.value

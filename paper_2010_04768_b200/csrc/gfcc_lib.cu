@@ -21,6 +21,7 @@
 #include "gfcc_gemm.cuh"
 #include "gfcc_kernels.cuh"
 #include "gfcc_solve.cuh"
+#include "gfcc_probe.cuh"
 
 using namespace gfcc;
 
@@ -839,6 +840,16 @@ extern "C" int gfcc_dgemm(void* stream, int M, int N, int K, double alpha, const
   if (K == 0) d.K0 = 0;
   cudaError_t e = launch_dgemm(d, (cudaStream_t)stream);
   return e == cudaSuccess ? GFCC_OK : GFCC_ECUDA;
+}
+
+extern "C" int gfcc_probe_fp64_peak(void* stream, int iters, int reps, double* tflops) {
+  if (!tflops || iters < 1 || reps < 1) return GFCC_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return GFCC_ECUDA; }
+  const double t = dmma_peak_probe((cudaStream_t)stream, iters, reps);
+  if (t < 0) return GFCC_ECUDA;
+  *tflops = t;
+  return GFCC_OK;
 }
 
 // ------------------------------------------------------------------------------------------
