@@ -92,8 +92,10 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *   "x0"           0: zero initial guess, 1: zeroth-order guess b/(omega - i eta + d) (default 1)
  *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3e9)
  *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256)
+ *   "overlap"      1: the K2 chain, the K4 chain and the small sigma terms run on three streams so that
+ *                  CTAs of one chain fill the ragged last wave of another; 0 (default): everything on the handle's stream
  *   "profile_gemm" 1: bracket every GEMM-engine launch with CUDA events on the handle's stream (statistics
- *                  "gemm_time_ms", "gemm_flops_timed", "gemm_launches_timed"); 0: off (default) */
+ *                  "gemm_time_ms", "gemm_flops_timed", "gemm_launches_timed"; implies overlap = 0 while it is on); 0: off (default) */
 int gfcc_set_option(gfcc_handle h, const char* key, double val);
 
 /* Statistics of the last call (double-valued): "iterations" (Arnoldi steps of the last solve),

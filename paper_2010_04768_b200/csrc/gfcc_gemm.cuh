@@ -330,6 +330,15 @@ inline int pick_wmf(int M, int wgm = gemm_wgm()) {
 }
 inline int gemm_bm(int M) { return gemm_wgm() * 8 * pick_wmf(M); }
 
+// engine selection: GFCC_GEMM_ENGINE=ws selects the warp-specialised kernel (gfcc_gemm_ws.cuh); the default is the
+// single-role kernel of this file until the ws kernel has passed the GPU parity suite (the WGM=4 variant implies v1).
+inline bool gemm_use_ws() {
+  static int w = -1;
+  if (w < 0) { const char* e = getenv("GFCC_GEMM_ENGINE"); w = (e && e[0] == 'w' && e[1] == 's') ? 1 : 0; }
+  return w == 1 && gemm_wgm() == 2;
+}
+cudaError_t launch_dgemm_ws(const GemmParams& p, bool a_kc, bool b_nc, bool sign, int wmf, cudaStream_t st);
+
 template <int WGM, int WMF, bool A_KC, bool B_NC, bool HAS_SIGN>
 inline cudaError_t launch_dgemm_t(const GemmParams& p, cudaStream_t st) {
   using T = GemmTile<WGM, WMF>;
@@ -394,6 +403,7 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   p.vecA = al16(d.A) && even(a_kc ? d.sAm : d.sAk0) && even(d.bsA) && (d.tabA ? d.tabs_even : even(d.sAk1));
   p.vecB = al16(d.B) && even(b_nc ? d.sBk0 : d.sBn) && even(d.bsB) && (d.tabB ? d.tabs_even : even(d.sBk1));
   const bool sign = d.sgn != nullptr;
+  if (gemm_use_ws()) return launch_dgemm_ws(p, a_kc, b_nc, sign, wmf, st);
   if (a_kc) return b_nc ? launch_dgemm_s<true, true>(sign, wgm, wmf, p, st) : launch_dgemm_s<true, false>(sign, wgm, wmf, p, st);
   return b_nc ? launch_dgemm_s<false, true>(sign, wgm, wmf, p, st) : launch_dgemm_s<false, false>(sign, wgm, wmf, p, st);
 }

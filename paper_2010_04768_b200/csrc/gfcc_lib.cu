@@ -19,6 +19,7 @@
 
 #include "../../include/gfcc.h"
 #include "gfcc_gemm.cuh"
+#include "gfcc_gemm_ws.cuh"
 #include "gfcc_kernels.cuh"
 #include "gfcc_solve.cuh"
 #include "gfcc_probe.cuh"
@@ -31,6 +32,9 @@ struct gfcc_ctx {
   int o = 0, v = 0, Q = 0, N = 0;
   long long npair = 0, ntri = 0, nvec = 0;   // nvec = o + npair*v (rows of an internal vector)
   cudaStream_t stream = 0;
+  cudaStream_t cur = 0;              // stream the next gemm()/kernel launch goes to (== stream outside sigma_internal)
+  cudaStream_t sB = nullptr, sC = nullptr;   // side streams: K4/V panel chain, small sigma terms (overlap with the K2 chain)
+  cudaEvent_t evFork = nullptr, evB = nullptr, evC = nullptr;
   std::string err;
   std::vector<void*> allocs;
   double bytes = 0;
@@ -45,12 +49,12 @@ struct gfcc_ctx {
   double* blk_sgn = nullptr;      // [o][o] +1 (i<n), -1 (i>n), 0 (i==n)
   // ---- workspace, sized for ws_nrhs ----
   int ws_nrhs = 0;
-  double *XU = nullptr, *Z = nullptr, *V = nullptr, *Y = nullptr, *KP = nullptr, *yv = nullptr, *part = nullptr, *d_omega = nullptr;
+  double *XU = nullptr, *Z = nullptr, *V = nullptr, *Y = nullptr, *KP = nullptr, *KP2 = nullptr, *yv = nullptr, *part = nullptr, *d_omega = nullptr;
   double *vin = nullptr, *vout = nullptr;   // internal vectors for gfcc_sigma_ip
   long long part_elems = 0;
   int panel_ni = 1;
   // ---- options / stats ----
-  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3e9, opt_max_batch = 256;
+  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3e9, opt_max_batch = 256, opt_overlap = 0;
   double st_iterations = 0, st_sigma_apps = 0, st_flops_sigma = 0, st_flops_create = 0, st_max_relres = 0, st_nunconv = 0;
   double st_gemm_launches = 0, st_kernel_launches = 0, st_flops_exec = 0;
   std::vector<double> last_relres;
@@ -104,11 +108,11 @@ static int gemm(gfcc_ctx* h, const GemmDesc& d) {
   const bool timed = h->prof && d.M > 0 && d.N > 0 && d.K0 > 0;
   if (timed) {
     while (h->ev_pool.size() < h->ev_used + 2) { cudaEvent_t e; CUDA_TRY(h, cudaEventCreate(&e)); h->ev_pool.push_back(e); }
-    CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used], h->stream));
+    CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used], h->cur));
   }
-  CUDA_TRY(h, launch_dgemm(d, h->stream));
+  CUDA_TRY(h, launch_dgemm(d, h->cur));
   if (timed) {
-    CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used + 1], h->stream));
+    CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used + 1], h->cur));
     h->ev_used += 2;
     h->ev_flops.push_back(2.0 * d.M * (double)d.N * (double)d.K1 * d.K0 * d.batch);
   }
@@ -144,7 +148,7 @@ static int gemm_splitk(gfcc_ctx* h, GemmDesc d, int S) {
     ++nparts;
   }
   const long long tot = (long long)d.M * d.N;
-  k_splitk_reduce<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(d.C, h->part, nparts, d.M, d.N, d.alpha, d.beta, d.sCm0,
+  k_splitk_reduce<<<(unsigned)((tot + 255) / 256), 256, 0, h->cur>>>(d.C, h->part, nparts, d.M, d.N, d.alpha, d.beta, d.sCm0,
                                                                       d.sCm1, d.Md > 0 ? d.Md : d.M, d.sCn0, d.sCn1,
                                                                       d.Nd > 0 ? d.Nd : d.N);
   KLAUNCH(h);
@@ -165,10 +169,11 @@ static void free_workspace(gfcc_ctx* h) {
   dev_free(h, h->XU, big); dev_free(h, h->Z, big); dev_free(h, h->V, big);
   dev_free(h, h->Y, (long long)h->Q * o * Nc);
   dev_free(h, h->KP, (long long)h->panel_ni * v * o * v);
+  dev_free(h, h->KP2, (long long)h->panel_ni * v * o * v);
   dev_free(h, h->yv, (long long)v * Nc);
   dev_free(h, h->d_omega, h->ws_nrhs);
   dev_free(h, h->vin, h->nvec * Nc); dev_free(h, h->vout, h->nvec * Nc);
-  h->XU = h->Z = h->V = h->Y = h->KP = h->yv = h->d_omega = h->vin = h->vout = nullptr;
+  h->XU = h->Z = h->V = h->Y = h->KP = h->KP2 = h->yv = h->d_omega = h->vin = h->vout = nullptr;
   h->ws_nrhs = 0;
 }
 
@@ -201,6 +206,7 @@ static int ensure_workspace(gfcc_ctx* h, int nrhs, bool need_abi_vecs) {
     TRY(dev_alloc(h, &h->XU, big)); TRY(dev_alloc(h, &h->Z, big)); TRY(dev_alloc(h, &h->V, big));
     TRY(dev_alloc(h, &h->Y, (long long)Q * o * Nc));
     TRY(dev_alloc(h, &h->KP, (long long)h->panel_ni * v * o * v));
+    if (h->opt_overlap != 0) TRY(dev_alloc(h, &h->KP2, (long long)h->panel_ni * v * o * v));
     TRY(dev_alloc(h, &h->yv, (long long)v * Nc));
     TRY(dev_alloc(h, &h->d_omega, nrhs));
   }
@@ -219,12 +225,22 @@ static int ensure_workspace(gfcc_ctx* h, int nrhs, bool need_abi_vecs) {
 static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double eta, const double* xin, double* sout) {
   const int o = h->o, v = h->v, Q = h->Q;
   const long long Nc = 2LL * nrhs, ld = (long long)o * Nc, ov = (long long)o * v;
-  cudaStream_t st = h->stream;
   const double* x2 = xin + (long long)o * Nc;
   double* s2 = sout + (long long)o * Nc;
+  // Three independent chains (the paper's "levelizer" exposes the same op-level parallelism):
+  //   A (handle stream): S7, then K2 panels -> Z        B (side stream): K4 panels -> V
+  //   C (side stream)  : sigma1, S6, S12, S5 -> sout
+  // Every GEMM CTA owns a whole SM, so running the chains on separate streams lets the block scheduler fill the
+  // ragged last wave of one panel GEMM with CTAs of another chain.  With per-launch GEMM timing on (profile_gemm)
+  // the chains are serialised on the handle's stream so that the event brackets do not overlap.
+  const bool par = h->opt_overlap != 0 && !h->prof && h->sB && h->sC && h->KP2;
+  cudaStream_t s0 = h->stream, sB = par ? h->sB : s0, sC = par ? h->sC : s0;
+  double* KPb = par ? h->KP2 : h->KP;
+  struct Restore { gfcc_ctx* h; ~Restore() { h->cur = h->stream; } } restore{h};
 
+  h->cur = s0;
   // XU[m][e][j][c] = x2[m,j,e]
-  k_unpack_xu<<<(unsigned)ov, 256, 0, st>>>(h->XU, xin, o, v, (int)Nc);
+  k_unpack_xu<<<(unsigned)ov, 256, 0, s0>>>(h->XU, xin, o, v, (int)Nc);
   KLAUNCH(h);
   // S1: Y[Q][(j,c)] = sum_(m,e) Lov[Q][(m,e)] XU[(m,e)][(j,c)]
   {
@@ -234,6 +250,11 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     d.C = h->Y; d.sCm0 = ld;
     TRY(gemm(h, d));
   }
+  if (par) {
+    CUDA_TRY(h, cudaEventRecord(h->evFork, s0));
+    CUDA_TRY(h, cudaStreamWaitEvent(sB, h->evFork, 0));
+    CUDA_TRY(h, cudaStreamWaitEvent(sC, h->evFork, 0));
+  }
   // S7: Z[(i,a)][(j,c)] = sum_Q Lm[Q][(i,a)] Y[Q][(j,c)]
   {
     GemmDesc d; d.M = (int)ov; d.N = (int)ld; d.K0 = Q;
@@ -242,9 +263,10 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     d.C = h->Z; d.sCm0 = ld;
     TRY(gemm(h, d));
   }
-  // S8+S9 (+S3,S4 folded): panels of K2'[(i,a)][(m,e)], Z -= K2' XU
   for (int i0 = 0; i0 < o; i0 += h->panel_ni) {
     const int ni = std::min(h->panel_ni, o - i0);
+    // ---- chain A: S8+S9 (+S3,S4 folded): panel of K2'[(i,a)][(m,e)], Z -= K2' XU
+    h->cur = s0;
     {
       GemmDesc d; d.M = ni * o; d.N = v * v; d.K0 = Q;
       d.A = h->LooT + (long long)i0 * o; d.sAm = 1; d.sAk0 = (long long)o * o;
@@ -252,7 +274,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
       d.C = h->KP; d.Md = o; d.sCm1 = (long long)v * ov; d.sCm0 = v; d.Nd = v; d.sCn1 = ov; d.sCn0 = 1;
       TRY(gemm(h, d));
     }
-    k_k2_fixup<<<(unsigned)(ni * v), 128, 0, st>>>(h->KP, h->Fmi, h->Fae, o, v, i0);
+    k_k2_fixup<<<(unsigned)(ni * v), 128, 0, s0>>>(h->KP, h->Fmi, h->Fae, o, v, i0);
     KLAUNCH(h);
     {
       GemmDesc d; d.M = ni * v; d.N = (int)ld; d.K0 = (int)ov;
@@ -262,35 +284,25 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
       d.alpha = -1.0; d.beta = 1.0;
       TRY(gemm(h, d));
     }
-  }
-  // S10: panels of K4[(n,f)][(m,e)] = sum_Q L[Q,m,f] L[Q,n,e];  V = K4 XU
-  for (int n0 = 0; n0 < o; n0 += h->panel_ni) {
-    const int nn = std::min(h->panel_ni, o - n0);
+    // ---- chain B: S10: panel of K4[(n,f)][(m,e)] = sum_Q L[Q,m,f] L[Q,n,e];  V = K4 XU
+    h->cur = sB;
     {
-      GemmDesc d; d.M = (int)ov; d.N = nn * v; d.K0 = Q;
+      GemmDesc d; d.M = (int)ov; d.N = ni * v; d.K0 = Q;
       d.A = h->Lov; d.sAm = 1; d.sAk0 = ov;
-      d.B = h->Lov + (long long)n0 * v; d.sBk0 = ov; d.sBn = 1;
-      d.C = h->KP; d.Md = v; d.sCm1 = v; d.sCm0 = ov; d.Nd = v; d.sCn1 = (long long)v * ov; d.sCn0 = 1;
+      d.B = h->Lov + (long long)i0 * v; d.sBk0 = ov; d.sBn = 1;
+      d.C = KPb; d.Md = v; d.sCm1 = v; d.sCm0 = ov; d.Nd = v; d.sCn1 = (long long)v * ov; d.sCn0 = 1;
       TRY(gemm(h, d));
     }
     {
-      GemmDesc d; d.M = nn * v; d.N = (int)ld; d.K0 = (int)ov;
-      d.A = h->KP; d.sAm = ov; d.sAk0 = 1;
+      GemmDesc d; d.M = ni * v; d.N = (int)ld; d.K0 = (int)ov;
+      d.A = KPb; d.sAm = ov; d.sAk0 = 1;
       d.B = h->XU; d.sBk0 = ld; d.sBn = 1;
-      d.C = h->V + (long long)n0 * v * ld; d.sCm0 = ld;
+      d.C = h->V + (long long)i0 * v * ld; d.sCm0 = ld;
       TRY(gemm(h, d));
     }
   }
-  // S11: Z[i][a][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]   (T2 blocks through the pair table, sign per block)
-  {
-    GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
-    d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
-    d.tabs_even = ((long long)v * v) % 2 == 0;
-    d.B = h->V; d.sBk1 = (long long)v * ld; d.sBk0 = ld; d.sBn = 1;
-    d.C = h->Z; d.sCm0 = ld; d.bsC = (long long)v * ld;
-    d.batch = o; d.beta = 1.0;
-    TRY(gemm(h, d));
-  }
+  // ---- chain C: everything that goes straight to sout ----
+  h->cur = sC;
   // S12a: yv[e][c] = - sum_(Q,m) Lov[Q][m][e] Y[Q][m][c]
   {
     GemmDesc d; d.M = v; d.N = (int)Nc; d.K1 = Q; d.K0 = o;
@@ -315,7 +327,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     d.C = sout; d.sCm0 = ld; d.alpha = -1.0; d.beta = 1.0;
     TRY(gemm_splitk(h, d, 32));
   }
-  k_sigma1_small<<<(unsigned)((o * nrhs + 127) / 128), 128, 0, st>>>(sout, xin, h->Fmi, d_omega, eta, o, nrhs);
+  k_sigma1_small<<<(unsigned)((o * nrhs + 127) / 128), 128, 0, sC>>>(sout, xin, h->Fmi, d_omega, eta, o, nrhs);
   KLAUNCH(h);
   // S6 (D): s2[(i<j)][(a,c)] = sum_(m<n) W[(i<j)][(m<n)] x2[(m<n)][(a,c)]
   {
@@ -341,8 +353,26 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     d.C = s2; d.sCm0 = Nc; d.beta = 1.0;
     TRY(gemm(h, d));
   }
+  // ---- join ----
+  h->cur = s0;
+  if (par) {
+    CUDA_TRY(h, cudaEventRecord(h->evB, sB));
+    CUDA_TRY(h, cudaEventRecord(h->evC, sC));
+    CUDA_TRY(h, cudaStreamWaitEvent(s0, h->evB, 0));
+    CUDA_TRY(h, cudaStreamWaitEvent(s0, h->evC, 0));
+  }
+  // S11: Z[i][a][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]   (T2 blocks through the pair table, sign per block)
+  {
+    GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
+    d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
+    d.tabs_even = ((long long)v * v) % 2 == 0;
+    d.B = h->V; d.sBk1 = (long long)v * ld; d.sBk0 = ld; d.sBn = 1;
+    d.C = h->Z; d.sCm0 = ld; d.bsC = (long long)v * ld;
+    d.batch = o; d.beta = 1.0;
+    TRY(gemm(h, d));
+  }
   // S13: shift + P(ij) ring
-  k_sigma2_epilogue<<<(unsigned)(h->npair * v), 64, 0, st>>>(sout, xin, h->Z, d_omega, eta, o, v, nrhs);
+  k_sigma2_epilogue<<<(unsigned)(h->npair * v), 64, 0, s0>>>(sout, xin, h->Z, d_omega, eta, o, v, nrhs);
   KLAUNCH(h);
   h->st_sigma_apps += 1;
   return GFCC_OK;
@@ -368,7 +398,13 @@ static int create_impl(gfcc_ctx* h, const double* fock, const double* T1, const 
   const int o = h->o, v = h->v, Q = h->Q, N = h->N;
   const long long ov = (long long)o * v, npair = h->npair, vv = (long long)v * v;
   cudaStream_t st = h->stream;
+  h->cur = st;
   const double flops0 = h->st_flops_exec;
+  CUDA_TRY(h, cudaStreamCreateWithFlags(&h->sB, cudaStreamNonBlocking));
+  CUDA_TRY(h, cudaStreamCreateWithFlags(&h->sC, cudaStreamNonBlocking));
+  CUDA_TRY(h, cudaEventCreateWithFlags(&h->evFork, cudaEventDisableTiming));
+  CUDA_TRY(h, cudaEventCreateWithFlags(&h->evB, cudaEventDisableTiming));
+  CUDA_TRY(h, cudaEventCreateWithFlags(&h->evC, cudaEventDisableTiming));
 
   TRY(dev_alloc(h, &h->Lov, Q * ov)); TRY(dev_alloc(h, &h->LooT, (long long)Q * o * o));
   TRY(dev_alloc(h, &h->Lvv, Q * vv)); TRY(dev_alloc(h, &h->Lm, Q * ov));
@@ -655,6 +691,15 @@ static int create_impl(gfcc_ctx* h, const double* fock, const double* T1, const 
   return GFCC_OK;
 }
 
+static void free_side_streams(gfcc_ctx* h) {
+  if (h->sB) { cudaStreamSynchronize(h->sB); cudaStreamDestroy(h->sB); }
+  if (h->sC) { cudaStreamSynchronize(h->sC); cudaStreamDestroy(h->sC); }
+  if (h->evFork) cudaEventDestroy(h->evFork);
+  if (h->evB) cudaEventDestroy(h->evB);
+  if (h->evC) cudaEventDestroy(h->evC);
+  h->sB = h->sC = nullptr; h->evFork = h->evB = h->evC = nullptr;
+}
+
 extern "C" int gfcc_create(int o, int v, int Q, const double* fock, const double* T1, const double* T2, const double* L1,
                            const double* L2, const double* Lchol, gfcc_handle* out) {
   if (out) *out = nullptr;
@@ -676,6 +721,7 @@ extern "C" int gfcc_create(int o, int v, int Q, const double* fock, const double
   int rc = create_impl(h, fock, T1, L1, Lchol);
   if (rc != GFCC_OK) {
     g_create_error = h->err;
+    free_side_streams(h);
     for (void* p : h->allocs) cudaFree(p);
     delete h;
     return rc;
@@ -687,6 +733,7 @@ extern "C" int gfcc_create(int o, int v, int Q, const double* fock, const double
 extern "C" int gfcc_destroy(gfcc_handle h) {
   if (!h) return GFCC_EINVAL;
   cudaStreamSynchronize(h->stream);
+  free_side_streams(h);
   solve_free(h->sw);
   for (void* p : h->allocs) cudaFree(p);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
@@ -699,6 +746,7 @@ extern "C" const char* gfcc_last_error(gfcc_handle h) { return h ? h->err.c_str(
 extern "C" int gfcc_set_stream(gfcc_handle h, void* s) {
   if (!h) return GFCC_EINVAL;
   h->stream = (cudaStream_t)s;
+  h->cur = h->stream;
   return GFCC_OK;
 }
 
@@ -711,6 +759,7 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "x0" && (val == 0 || val == 1)) h->opt_x0 = val;
   else if (k == "panel_bytes" && val > 0) { h->opt_panel_bytes = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
+  else if (k == "overlap" && (val == 0 || val == 1)) { h->opt_overlap = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "profile_gemm") { h->prof = (val != 0); h->ev_used = 0; h->ev_flops.clear(); }
   else { h->err = "gfcc_set_option: unknown key or invalid value: " + k; return GFCC_EINVAL; }
   return GFCC_OK;
