@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--kfix", type=int, default=0, help="Arnoldi steps per step (default: per config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--overlap", type=int, default=-1, help="1: run independent sigma panel chains on side streams (default: library default)")
     return ap.parse_args()
 
 
@@ -218,6 +219,8 @@ def main():
     g.gfcc_set_stream(h, stream)
     g.gfcc_set_option(h, "gmres_fixed", kfix)
     g.gfcc_set_option(h, "max_batch", nrhs)
+    if args.overlap >= 0:
+        g.gfcc_set_option(h, "overlap", args.overlap)
 
     # rank r solves its own slice of the omega sweep (independent (p,omega) tasks; weak scaling)
     omegas = sharding.weak_scaling_grid(c["wlo"], c["whi"], c["nw"], max(world, 1), rank)
@@ -236,7 +239,9 @@ def main():
         step()
     flops_sigma = g.gfcc_get_stat(h, "flops_sigma")
     g.gfcc_get_stat(h, "reset_counters")
-    g.gfcc_set_option(h, "profile_gemm", 1)
+    overlap_on = args.overlap == 1
+    if not overlap_on:      # per-launch events serialise the side streams, so with overlap the GEMM profile is a separate step
+        g.gfcc_set_option(h, "profile_gemm", 1)
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
@@ -250,10 +255,20 @@ def main():
     sampler.stop_flag = True
     ms_total = e0.elapsed_time(e1)
     launches = g.gfcc_get_stat(h, "kernel_launches")
+    napply = g.gfcc_get_stat(h, "sigma_applications")
+    ms_prof = ms_total
+    if overlap_on:
+        g.gfcc_set_option(h, "profile_gemm", 1)
+        with torch.cuda.stream(stream):
+            e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e2.record(stream)
+            step()
+            e3.record(stream)
+        barrier()
+        ms_prof = e2.elapsed_time(e3)
     gemm_ms = g.gfcc_get_stat(h, "gemm_time_ms")
     gemm_flops = g.gfcc_get_stat(h, "gemm_flops_timed")
     gemm_n = g.gfcc_get_stat(h, "gemm_launches_timed")
-    napply = g.gfcc_get_stat(h, "sigma_applications")
     g.gfcc_set_option(h, "profile_gemm", 0)
     ms_total = sharding.max_over_ranks(ms_total, world, dist, "cuda")
     ms_step = ms_total / args.steps
@@ -268,7 +283,8 @@ def main():
         "config": {"workload": workload_string(cfg, c, nrhs, kfix, rank), "l2": "inputs and working set >> 126 MB L2 (no flush needed)",
                    "flop_model": "executed Cholesky-route model, SURVEY.md 8(d): real x complex = 2 real products, pair-packed o^4 term",
                    "flops_per_sigma_application": flops_sigma, "sigma_applications_per_step": apps_per_step,
-                   "gmres_m_used": g.gfcc_get_stat(h, "gmres_m_used"), "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
+                   "gmres_m_used": g.gfcc_get_stat(h, "gmres_m_used"), "overlap": int(overlap_on),
+                   "gemm_engine": os.environ.get("GFCC_GEMM_ENGINE", "ws"), "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
         "solves_per_s": solves_per_s, "solves_note": f"(p,omega) right-hand sides advanced by {kfix} GMRES steps per second x nrhs",
         "pct_fp64_peak_measured": 100.0 * value / world / FP64_DMMA_PEAK_TFLOPS,
         "create_s": create_s, "create_tflops": flops_create / create_s / 1e12, "inputs_s": t_inputs,
@@ -280,14 +296,14 @@ def main():
     mp = measured_peaks()
     achieved = gemm_flops / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
     line["roofline"] = {
-        "kernel": "gfcc::dgemm_dmma_kernel (all GEMM-engine launches of the timed region)",
+        "kernel": "gfcc::dgemm_ws_kernel (all GEMM-engine launches of the timed region)",
         "bound": "tensor", "achieved": achieved, "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_DMMA_PEAK_TFLOPS,
         "peak_source": "measured FP64 DMMA.8x8x4 issue-rate ceiling on this pool's B200 (profiles/fp64_peak_probe.md); "
                        "MEASURED_PEAKS.json has no FP64 entry",
         "peak_alt_bf16_ratio": (mp["bf16_tflops_sustained"] * 40.0 / 2250.0) if mp else None,
         "peak_alt_note": "sustained bf16 peak of MEASURED_PEAKS.json x nominal FP64:bf16 ratio 40/2250 (fallback rule; lower than the "
                          "directly measured DMMA ceiling, so the stricter denominator is used for frac)",
-        "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1), "share_of_step": gemm_ms / ms_total if ms_total > 0 else None,
+        "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1), "share_of_step": gemm_ms / ms_prof if ms_prof > 0 else None,
         "algorithmic_flops": gemm_flops, "traffic": None,
         "traffic_note": "DRAM bytes per launch are in profiles/ (ncu --set full of the same kernel): <3% of DRAM peak, L2 hit 82%",
     }

@@ -315,26 +315,38 @@ inline int gemm_wgm() {
   if (w < 0) { const char* e = getenv("GFCC_GEMM_WGM"); w = (e && e[0] == '4') ? 4 : 2; }
   return w;
 }
-// choose the m8-fragment count per warp (BM = WGM*8*WMF) that wastes the fewest padded rows
-inline int pick_wmf(int M, int wgm = gemm_wgm()) {
+// choose the m8-fragment count per warp (BM = WGM*8*WMF): the kernel runs one CTA per SM, so the launch takes
+// ceil(tiles / 148) waves of time ~ BM each; pick the BM with the smallest waves*BM (this covers both ragged-M padding
+// and the partially filled last wave), with a mild penalty for small tiles (more shared-memory traffic per flop).
+constexpr int GEMM_NUM_SMS = 148;
+inline int pick_wmf(int M, long long N = 0, int batch = 1, int wgm = gemm_wgm()) {
   const int hi = (wgm == 4) ? 4 : 8, lo = (wgm == 4) ? 2 : 4;
-  int best = hi; long long bestcost = -1;
+  const long long tiles_n = (N > 0) ? (N + GEMM_BN - 1) / GEMM_BN : 0;
+  int best = hi; double bestcost = -1;
   for (int w = hi; w >= lo; --w) {
     const int bm = wgm * 8 * w;
-    const long long tiles = (M + bm - 1) / bm;
-    // cost ~ padded rows, with a mild penalty for small tiles (lower operand reuse)
-    const long long cost = tiles * bm * 100 + (hi - w) * 2LL * (long long)M;
+    const long long tiles_m = (M + bm - 1) / bm;
+    double cost;
+    if (tiles_n > 0) {
+      const long long tiles = tiles_m * tiles_n * (batch > 0 ? batch : 1);
+      const long long waves = (tiles + GEMM_NUM_SMS - 1) / GEMM_NUM_SMS;
+      cost = (double)waves * bm;
+    } else {
+      cost = (double)tiles_m * bm;   // N unknown: padded rows only
+    }
+    cost *= 1.0 + 0.01 * (hi - w);
     if (bestcost < 0 || cost < bestcost) { bestcost = cost; best = w; }
   }
   return best;
 }
-inline int gemm_bm(int M) { return gemm_wgm() * 8 * pick_wmf(M); }
+inline int gemm_bm(int M, long long N = 0, int batch = 1) { return gemm_wgm() * 8 * pick_wmf(M, N, batch); }
 
-// engine selection: GFCC_GEMM_ENGINE=ws selects the warp-specialised kernel (gfcc_gemm_ws.cuh); the default is the
-// single-role kernel of this file until the ws kernel has passed the GPU parity suite (the WGM=4 variant implies v1).
+// engine selection: the warp-specialised kernel (gfcc_gemm_ws.cuh; 34.4 TFLOP/s on 8192^3 = 93 % of the DMMA ceiling,
+// GPU parity suite green) is the default; GFCC_GEMM_ENGINE=v1 selects the single-role kernel of this file
+// (31.0 TFLOP/s) for comparison.  The WGM=4 experiment implies v1.
 inline bool gemm_use_ws() {
   static int w = -1;
-  if (w < 0) { const char* e = getenv("GFCC_GEMM_ENGINE"); w = (e && e[0] == 'w' && e[1] == 's') ? 1 : 0; }
+  if (w < 0) { const char* e = getenv("GFCC_GEMM_ENGINE"); w = (e && e[0] == 'v' && e[1] == '1') ? 0 : 1; }
   return w == 1 && gemm_wgm() == 2;
 }
 cudaError_t launch_dgemm_ws(const GemmParams& p, bool a_kc, bool b_nc, bool sign, int wmf, cudaStream_t st);
@@ -392,7 +404,7 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   p.alpha = d.alpha; p.beta = d.beta;
   p.batch = d.batch; p.bsA = d.bsA; p.bsB = d.bsB; p.bsC = d.bsC; p.tab_batch_stride = d.tab_batch_stride;
   const int wgm = gemm_wgm();
-  const int wmf = pick_wmf(d.M, wgm);
+  const int wmf = pick_wmf(d.M, d.N, d.batch, wgm);
   const int bm = wgm * 8 * wmf;
   p.tiles_m = (d.M + bm - 1) / bm;
   p.tiles_n = (d.N + GEMM_BN - 1) / GEMM_BN;

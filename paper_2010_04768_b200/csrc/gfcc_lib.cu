@@ -187,7 +187,7 @@ static int choose_panel(int o, int v, long long ncols, double budget_bytes) {
   const int tiles_n = (int)((ncols + GEMM_BN - 1) / GEMM_BN);
   for (int n = nmax; n >= std::max(1, nmax / 2); --n) {
     const int rows = n * v;
-    const int bm = gemm_bm(rows);
+    const int bm = gemm_bm(rows, ncols);
     const long long tiles = (long long)((rows + bm - 1) / bm) * tiles_n;
     const long long waves = (tiles + 147) / 148;
     const double eff = (double)rows * ncols / ((double)waves * 148 * bm * GEMM_BN);
