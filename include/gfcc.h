@@ -112,6 +112,30 @@ int gfcc_get_residuals(gfcc_handle h, int n, double* relres, int* iters);
  *   "Lm" [Q][o][v].  Returns the element count (>0), or <0 on error; out may be NULL to query size.   */
 long long gfcc_get_intermediate(gfcc_handle h, const char* name, double* out);
 
+/* ---- Model-order reduction (Eq. 9-10, Alg. 1 lines 18-21 PAPER.md:225-228) ----
+ * The subspace S = {v_1..v_m} is a REAL orthonormal basis in the packed 1h + 2h1p(i<j) metric, owned by the handle
+ * (Eq. 10 writes transposes and Hbar, b, c are real: every complex X contributes Re X and Im X; reading 24).
+ *
+ * gfcc_mor_reset : (re)allocate an empty subspace with room for m_cap vectors (rounded up to even, at most the
+ *   dimension o + o(o-1)/2*v); m_cap = 0 frees it.  Device memory: 2*n*m_cap + m_cap^2 doubles.
+ * gfcc_mor_extend: Gram-Schmidt (Alg. 1 line 18) of nx new solutions X1 [nx][o], X2 [nx][o][o][v] (device, complex,
+ *   layouts of gfcc_sigma_ip, e.g. the output of gfcc_solve_ip_x) against S, in the order Re X_0, Im X_0, Re X_1, ...;
+ *   each candidate is normalised, orthogonalised twice (classical Gram-Schmidt with re-orthogonalisation) and DROPPED
+ *   if what is left of its unit norm is <= droptol (or if the subspace is full); then the projection (line 19):
+ *   Hbar*v for the accepted vectors by batched sigma at omega = eta = 0 and H^ = S^T Hbar S (new rows and columns).
+ *   *m_out [host, nullable] receives the new dimension m.  Synchronous.
+ * gfcc_mor_solve : b^ = S^T b_p, c^ = S^T c_q (q over the same list), then for every omega[iw] of the (fine) grid the
+ *   reduced system (omega - i eta + H^) X^ = b^ by dense complex LU with partial pivoting (one CTA per frequency),
+ *   G[iw][ip][iq] = c^_q^T X^_p  complex [nw][np][np]  and  A[iw] = (1/pi) sum_p Im G[iw][p][p]  (Eq. 9; sign: DESIGN.md
+ *   reading 25).  p, omega host; G and A (nullable) may be host or device pointers.  Returns GFCC_ENOCONV if a reduced
+ *   matrix is exactly singular.  Synchronous.
+ * gfcc_mor_get   : parity hooks.  "m", "cap" return the value; "Hhat" [m][m], "S" [n][m], "HS" (= Hbar S) [n][m] are
+ *   copied to `out` (host or device; NULL queries the element count).  Returns the count or a negative error code.    */
+int gfcc_mor_reset(gfcc_handle h, int m_cap);
+int gfcc_mor_extend(gfcc_handle h, int nx, const void* X1, const void* X2, double droptol, int* m_out);
+int gfcc_mor_solve(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, void* G, double* A);
+long long gfcc_mor_get(gfcc_handle h, const char* name, double* out);
+
 const char* gfcc_last_error(gfcc_handle h);
 int gfcc_destroy(gfcc_handle h);
 

@@ -23,7 +23,8 @@ GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 
 EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_intermediate", "gfcc_last_error",
-           "gfcc_destroy", "gfcc_dgemm", "gfcc_probe_fp64_peak"]
+           "gfcc_destroy", "gfcc_dgemm", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
+           "gfcc_mor_get"]
 
 
 class GfccError(RuntimeError):
@@ -62,8 +63,13 @@ def lib():
     L.gfcc_destroy.argtypes = [vp]
     L.gfcc_dgemm.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll]
     L.gfcc_probe_fp64_peak.argtypes = [vp, ci, ci, dp]
+    L.gfcc_mor_reset.argtypes = [vp, ci]
+    L.gfcc_mor_extend.argtypes = [vp, ci, vp, vp, cd, ip]
+    L.gfcc_mor_solve.argtypes = [vp, ci, ip, ci, dp, cd, vp, dp]
+    L.gfcc_mor_get.argtypes = [vp, ctypes.c_char_p, vp]
+    L.gfcc_mor_get.restype = cll
     for name in EXPORTS:
-        if name not in ("gfcc_get_intermediate", "gfcc_last_error"):
+        if name not in ("gfcc_get_intermediate", "gfcc_last_error", "gfcc_mor_get"):
             getattr(L, name).restype = ci
     _lib = L
     return L
@@ -245,3 +251,46 @@ def gfcc_probe_fp64_peak(iters=20000, reps=5, stream=0):
     if rc != GFCC_OK:
         raise GfccError(rc, "gfcc_probe_fp64_peak failed")
     return out.value
+
+
+# ---- model-order reduction (Eq. 9-10; Alg. 1 lines 18-21) -----------------------------------
+def gfcc_mor_reset(h, m_cap):
+    _check(h, lib().gfcc_mor_reset(h.ptr, int(m_cap)))
+
+
+def gfcc_mor_extend(h, X1, X2, droptol=1e-8):
+    """X1 [nx,o], X2 [nx,o,o,v] complex128 CUDA tensors (e.g. from gfcc_solve_ip(..., return_x=True)) -> new dimension m."""
+    torch = _torch()
+    m = ctypes.c_int(0)
+    _check(h, lib().gfcc_mor_extend(h.ptr, int(X1.shape[0]), _dev(X1, torch.complex128), _dev(X2, torch.complex128),
+                                    float(droptol), ctypes.byref(m)))
+    return m.value
+
+
+def gfcc_mor_solve(h, p, omega, eta):
+    """Reduced model on a frequency grid -> (G [nw,np,np] complex128, A [nw] float64), host numpy arrays."""
+    _torch()
+    pa = np.ascontiguousarray(p, dtype=np.int32)
+    om = np.ascontiguousarray(np.atleast_1d(omega), dtype=np.float64)
+    G = np.empty((len(om), len(pa), len(pa)), dtype=np.complex128)
+    A = np.empty(len(om), dtype=np.float64)
+    _check(h, lib().gfcc_mor_solve(h.ptr, len(pa), pa.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), len(om),
+                                   om.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), float(eta), G.ctypes.data,
+                                   A.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+    return G, A
+
+
+def gfcc_mor_get(h, name):
+    """"m"/"cap" -> int; "Hhat" -> [m,m], "S"/"HS" -> [n,m] host numpy arrays (parity hooks)."""
+    n = lib().gfcc_mor_get(h.ptr, name.encode(), None)
+    if n < 0:
+        _check(h, int(n))
+    if name in ("m", "cap"):
+        return int(n)
+    m = int(lib().gfcc_mor_get(h.ptr, b"m", None))
+    out = np.empty(int(n), dtype=np.float64)
+    if n > 0:
+        n2 = lib().gfcc_mor_get(h.ptr, name.encode(), out.ctypes.data)
+        if n2 < 0:
+            _check(h, int(n2))
+    return out.reshape(-1, m) if m > 0 else out.reshape(0, 0)

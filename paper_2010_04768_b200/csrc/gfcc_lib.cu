@@ -23,6 +23,7 @@
 #include "gfcc_kernels.cuh"
 #include "gfcc_solve.cuh"
 #include "gfcc_probe.cuh"
+#include "gfcc_mor.cuh"
 
 using namespace gfcc;
 
@@ -60,6 +61,11 @@ struct gfcc_ctx {
   std::vector<double> last_relres;
   std::vector<int> last_iters;
   SolveWs sw;
+  // ---- MOR subspace: S, Hbar*S as [n_pad][cap] real, H^ as [cap][cap] ----
+  int mor_cap = 0, mor_m = 0;
+  long long mor_npad = 0;
+  double *mor_S = nullptr, *mor_HS = nullptr, *mor_Hh = nullptr;
+  double st_mor_dropped = 0, st_mor_sigma_cols = 0;
   // ---- optional per-launch timing of the GEMM engine (CUDA events on the handle's stream; bench.py roofline) ----
   bool prof = false;
   std::vector<cudaEvent_t> ev_pool;
@@ -983,3 +989,5 @@ extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, cons
 extern "C" int gfcc_solve_ip(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol, void* G) {
   return gfcc_solve_ip_x(h, np, p, nw, omega, eta, tol, G, nullptr, nullptr);
 }
+
+#include "gfcc_mor_host.inl"
