@@ -32,6 +32,7 @@ import numpy as np  # noqa: E402
 FP64_DMMA_PEAK_TFLOPS = 36.95   # measured on this pool's B200: DMMA.8x8x4 issue-rate probe (profiles/fp64_peak_probe.md)
 KFIX = {0: 20, 1: 8, 2: 4, 3: 2, 4: 1}      # Arnoldi steps per timed step (bounded so that a default run ends in minutes)
 DEFAULT_CONFIG = 4
+NCU_TRAFFIC_BYTES = {4: 44.098195e9 + 0.131195e9}   # profiles/r1_gemm_ws_ncu_full.md, launch 7
 
 
 def parse():
@@ -44,6 +45,10 @@ def parse():
     ap.add_argument("--kfix", type=int, default=0, help="Arnoldi steps per step (default: per config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-baseline-only", action="store_true",
+                    help="(internal) child process of the default run: time the oracle sample, print its JSON, exit")
+    ap.add_argument("--cpu-baseline-serial", action="store_true",
+                    help="time the oracle AFTER the GPU part on all host cores instead of beside it (doubles the run time at config 4)")
     ap.add_argument("--overlap", type=int, default=-1, help="1: run independent sigma panel chains on side streams (default: library default)")
     return ap.parse_args()
 
@@ -93,7 +98,7 @@ def workload_string(cfg, c, nrhs, kfix, rank_shift):
 
 
 # ---------------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, c, nsamp, nrhs_s, threads_note=True):
+def oracle_sample(cfg, c, nsamp, nrhs_s, ready_cb=None):
     """time the CPU oracle (as it stands) on a bounded sample of the workload; returns (seconds, description, cores)."""
     import torch
     import gfcc_inputs as gi
@@ -107,9 +112,9 @@ def oracle_sample(cfg, c, nsamp, nrhs_s, threads_note=True):
     del s
     if dev == "cuda":
         torch.cuda.empty_cache()
+    if ready_cb is not None:
+        ready_cb()
     w = np.linspace(c["wlo"], c["whi"], nrhs_s)
-    if cfg <= 1 and False:
-        pass
     t0 = time.time()
     orc = oracle.Oracle(o, v, Q, host["fock"], host["T1"], host["T2p"], host["L1"], host["L2p"], host["Lchol"], oracle.MODE_ROWS)
     t_setup = time.time() - t0
@@ -121,17 +126,71 @@ def oracle_sample(cfg, c, nsamp, nrhs_s, threads_note=True):
     return t_setup, t_rows, trip, oracle.threads()
 
 
-def cpu_baseline(cfg, c, nrhs, flops_sigma):
+def cpu_baseline(cfg, c, nrhs, flops_sigma, ready_cb=None):
     nsamp, nrhs_s = (4, 2) if cfg <= 2 else ((2, 1) if cfg == 3 else (1, 1))
-    t_setup, t_rows, trip, cores = oracle_sample(cfg, c, nsamp, nrhs_s)
+    t_setup, t_rows, trip, cores = oracle_sample(cfg, c, nsamp, nrhs_s, ready_cb)
     npair = c["o"] * (c["o"] - 1) // 2
     rows_total = npair * c["v"] * nrhs
     t_full = t_rows * rows_total / (nsamp * nrhs_s)      # linear extrapolation to all rows of all RHS
-    return {"value": flops_sigma / t_full / 1e12, "unit": "TFLOP/s", "cores": cores, "kind": "oracle",
+    return {"seconds_full": t_full, "value": flops_sigma / t_full / 1e12, "unit": "TFLOP/s", "cores": cores, "kind": "oracle",
             "sample": (f"row-sampled oracle sigma (oracle/gfcc_oracle.cpp orc_sigma_rows): {nsamp} sigma2 rows + 1 sigma1 row x {nrhs_s} "
                        f"RHS of config {cfg} in {t_rows:.1f} s (+{t_setup:.1f} s one-time dressing), EXTRAPOLATED linearly to the "
                        f"{rows_total} (row,RHS) outputs of one batched application"),
             "seconds_sample": t_rows, "seconds_setup": t_setup}
+
+
+def model_flops(c, nrhs):
+    """executed flop model of one batched sigma application; the library reports the same
+    number as gfcc_get_stat(h, "flops_sigma")."""
+    o, v, Q = c["o"], c["v"], c["Q"]
+    npair = o * (o - 1) // 2
+    Nc = 2.0 * nrhs
+    ov = o * v
+    return (2 * Q * ov * o * Nc * 2 + 4 * Q * ov * ov + 6 * ov * ov * o * Nc + 2 * npair * npair * v * Nc
+            + 2 * npair * v * v * Nc + 2 * npair * v * o * Nc + 2 * Q * o * v * Nc + 2 * Q * o * o * Nc + 2 * ov * o * Nc)
+
+
+def run_cpu_baseline_child(args):
+    """child of the default run: generates its own copy of the inputs (on the GPU when there is one, then moved to the
+    host and the device memory released), prints READY, times the oracle sample, prints one JSON line."""
+    import gfcc_inputs as gi
+    c = gi.CONFIGS[args.config]
+    nrhs = c["np"] * c["nw"]
+    cb = cpu_baseline(args.config, c, nrhs, model_flops(c, nrhs), ready_cb=lambda: print("READY", flush=True))
+    print(json.dumps(cb), flush=True)
+    return 0
+
+
+def start_cpu_baseline_child(cfg):
+    """start the oracle timing BESIDE the GPU part (the GPU part is timed on the device with CUDA events and its launches
+    are 10-300 ms long, so host contention does not reach it); the oracle gets all host cores but two."""
+    cores = os.cpu_count() or 4
+    env = dict(os.environ)
+    env["OMP_NUM_THREADS"] = str(max(1, cores - 2))
+    child = subprocess.Popen([sys.executable, os.path.abspath(__file__), "--cpu-baseline-only", "--config", str(cfg)],
+                             stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, env=env)
+    while True:                                   # wait until the child has released the device memory of its inputs
+        ln = child.stdout.readline()
+        if not ln or ln.strip() == "READY":
+            break
+    return child
+
+
+def finish_cpu_baseline_child(child, flops_sigma, timeout_s=900):
+    try:
+        out, _ = child.communicate(timeout=timeout_s)
+    except subprocess.TimeoutExpired:
+        child.kill()
+        return {"value": None, "unit": "TFLOP/s", "cores": None, "kind": "oracle", "sample": f"oracle sample not finished after {timeout_s} s"}
+    for ln in reversed(out.strip().splitlines()):
+        if ln.startswith("{"):
+            cb = json.loads(ln)
+            cb["value"] = flops_sigma / cb.pop("seconds_full") / 1e12
+            cb["sample"] += "; timed in a child process BESIDE the GPU part of this run (OMP threads = host cores - 2)"
+            cb.pop("seconds_sample", None)
+            cb.pop("seconds_setup", None)
+            return cb
+    return {"value": None, "unit": "TFLOP/s", "cores": None, "kind": "oracle", "sample": "oracle child printed no result"}
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -147,10 +206,7 @@ def run_reference(args):
     kfix = args.kfix or KFIX[cfg]
     o, v, Q = c["o"], c["v"], c["Q"]
     npair = o * (o - 1) // 2
-    Nc = 2.0 * nrhs
-    ov = o * v
-    flops_sigma = (2 * Q * ov * o * Nc * 2 + 4 * Q * ov * ov + 6 * ov * ov * o * Nc + 2 * npair * npair * v * Nc
-                   + 2 * npair * v * v * Nc + 2 * npair * v * o * Nc + 2 * Q * o * v * Nc + 2 * Q * o * o * Nc + 2 * ov * o * Nc)
+    flops_sigma = model_flops(c, nrhs)
     vals = []
     last = None
     for it in range(args.warmup + args.steps):
@@ -178,6 +234,8 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------------
 def main():
     args = parse()
+    if args.cpu_baseline_only:
+        return run_cpu_baseline_child(args)
     if args.impl == "reference":
         return run_reference(args)
 
@@ -202,6 +260,11 @@ def main():
     o, v, Q = c["o"], c["v"], c["Q"]
     nrhs = c["np"] * c["nw"]
     kfix = args.kfix or KFIX[cfg]
+
+    # ---- CPU baseline: started first, runs beside the GPU part (rank 0, N = 1 only) ----
+    cpu_child = None
+    if world == 1 and not args.no_cpu_baseline and not args.cpu_baseline_serial:
+        cpu_child = start_cpu_baseline_child(cfg)
 
     # ---- inputs (seeded, generated directly in HBM) and one-time intermediates ----
     t0 = time.time()
@@ -304,8 +367,11 @@ def main():
         "peak_alt_note": "sustained bf16 peak of MEASURED_PEAKS.json x nominal FP64:bf16 ratio 40/2250 (fallback rule; lower than the "
                          "directly measured DMMA ceiling, so the stricter denominator is used for frac)",
         "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1), "share_of_step": gemm_ms / ms_prof if ms_prof > 0 else None,
-        "algorithmic_flops": gemm_flops, "traffic": None,
-        "traffic_note": "DRAM bytes per launch are in profiles/ (ncu --set full of the same kernel): <3% of DRAM peak, L2 hit 82%",
+        "algorithmic_flops": gemm_flops, "traffic": NCU_TRAFFIC_BYTES.get(cfg),
+        "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel from ncu --set full "
+                        "(profiles/r1_gemm_ws_ncu_full.md): the config-4 S9 panel GEMM 2640 x 5760 x 118800 (the most frequent big launch of a "
+                        "step), whose algorithmic bytes (A + B + C once) are 8.2e9; DRAM is 4.9 % busy in that launch (tensor-bound, 91.7 % DMMA "
+                        "pipe), L2 hit 80 %; null for configs without a capture",
     }
 
     # ---- end to end through the C ABI with HOST buffers: one batched sigma application, copies inside the call ----
@@ -318,7 +384,7 @@ def main():
             torch.cuda.empty_cache()
             wr = np.repeat(omegas, c["np"])[:nrhs] if len(omegas) * c["np"] >= nrhs else np.resize(omegas, nrhs)
             g.gfcc_sigma_ip_host(h, wr, c["eta"], X1h.numpy(), X2h.numpy())   # warm-up
-            nrep = 2 if cfg >= 3 else 3
+            nrep = 1 if cfg >= 3 else 3
             t0 = time.perf_counter()
             for _ in range(nrep):
                 S1h, S2h = g.gfcc_sigma_ip_host(h, wr, c["eta"], X1h.numpy(), X2h.numpy())
@@ -334,11 +400,13 @@ def main():
     torch.cuda.empty_cache()
 
     # ---- CPU baseline: the oracle on the host cores, bounded sample (rank 0, N = 1 only) ----
-    if world == 1 and not args.no_cpu_baseline:
+    if cpu_child is not None:
+        line["cpu_baseline"] = finish_cpu_baseline_child(cpu_child, flops_sigma)
+    elif world == 1 and not args.no_cpu_baseline:
         try:
             cb = cpu_baseline(cfg, c, nrhs, flops_sigma)
-            cb.pop("seconds_sample", None)
-            cb.pop("seconds_setup", None)
+            for k in ("seconds_sample", "seconds_setup", "seconds_full"):
+                cb.pop(k, None)
             line["cpu_baseline"] = cb
         except Exception as ex:   # noqa: BLE001
             line["cpu_baseline"] = {"value": None, "unit": "TFLOP/s", "cores": None, "kind": "oracle", "sample": f"failed: {str(ex)[:200]}"}

@@ -24,6 +24,7 @@
 #include "gfcc_solve.cuh"
 #include "gfcc_probe.cuh"
 #include "gfcc_mor.cuh"
+#include "gfcc_ozaki.cuh"
 
 using namespace gfcc;
 
@@ -895,6 +896,54 @@ extern "C" int gfcc_dgemm(void* stream, int M, int N, int K, double alpha, const
   if (K == 0) d.K0 = 0;
   cudaError_t e = launch_dgemm(d, (cudaStream_t)stream);
   return e == cudaSuccess ? GFCC_OK : GFCC_ECUDA;
+}
+
+// FP64-accurate GEMM on the INT8 tensor pipe (gfcc_ozaki.cuh): C = alpha*A*B + beta*C, same operand
+// conventions as gfcc_dgemm.  Synchronous; temporary slices are allocated and freed inside.  ms_slice / ms_gemm (nullable)
+// receive the CUDA-event times of the slicing pass and of the tensor-core kernel.
+extern "C" int gfcc_dgemm_ozaki(void* stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
+                                const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn,
+                                int nslices, double* ms_slice, double* ms_gemm) {
+  if (M < 1 || N < 1 || K < 1 || !A || !B || !C || nslices < 1 || nslices > OZ_MAX_SLICES) return GFCC_EINVAL;
+  if ((sAm != 1 && sAk != 1) || (sBk != 1 && sBn != 1)) return GFCC_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  OzOperand a, b;
+  a.base = A; a.sR = sAm; a.sK0 = sAk; a.R = M; a.K0 = K;
+  b.base = B; b.sR = sBn; b.sK0 = sBk; b.R = N; b.K0 = K;
+  OzSliced sa, sb;
+  oz_shape(sa, M, K, nslices); oz_shape(sb, N, K, nslices);
+  int* fail = nullptr;
+  cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+  int rc = GFCC_OK;
+  auto cleanup = [&]() {
+    cudaFree(sa.q); cudaFree(sa.scale); cudaFree(sa.amax); cudaFree(sb.q); cudaFree(sb.scale); cudaFree(sb.amax); cudaFree(fail);
+    for (auto e : ev) if (e) cudaEventDestroy(e);
+  };
+  do {
+    if (cudaMalloc(&sa.q, sa.bytes()) != cudaSuccess || cudaMalloc(&sb.q, sb.bytes()) != cudaSuccess ||
+        cudaMalloc(&sa.scale, (size_t)M * 8) != cudaSuccess || cudaMalloc(&sb.scale, (size_t)N * 8) != cudaSuccess ||
+        cudaMalloc(&sa.amax, (size_t)M * 8) != cudaSuccess || cudaMalloc(&sb.amax, (size_t)N * 8) != cudaSuccess ||
+        cudaMalloc(&fail, sizeof(int)) != cudaSuccess) { rc = GFCC_ENOMEM; break; }
+    for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    if (rc) break;
+    cudaMemsetAsync(fail, 0, sizeof(int), st);
+    cudaEventRecord(ev[0], st);
+    if (oz_slice(a, sa, st) != cudaSuccess || oz_slice(b, sb, st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    cudaEventRecord(ev[1], st);
+    OzCDesc c; c.C = C; c.sCm0 = sCm; c.sCn0 = sCn; c.alpha = alpha; c.beta = beta;
+    if (oz_igemm(sa, sb, c, fail, st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    cudaEventRecord(ev[2], st);
+    if (cudaStreamSynchronize(st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    int hfail = 0;
+    cudaMemcpy(&hfail, fail, sizeof(int), cudaMemcpyDeviceToHost);
+    if (hfail) { rc = GFCC_ECUDA; break; }
+    float t = 0;
+    if (ms_slice) { cudaEventElapsedTime(&t, ev[0], ev[1]); *ms_slice = t; }
+    if (ms_gemm) { cudaEventElapsedTime(&t, ev[1], ev[2]); *ms_gemm = t; }
+  } while (0);
+  if (rc != GFCC_OK) cudaGetLastError();
+  cleanup();
+  return rc;
 }
 
 extern "C" int gfcc_probe_fp64_peak(void* stream, int iters, int reps, double* tflops) {

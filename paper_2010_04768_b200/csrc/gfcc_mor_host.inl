@@ -197,12 +197,12 @@ extern "C" int gfcc_mor_solve(gfcc_handle h, int np, const int* p, int nw, const
   {
     static bool attr_set = false;
     if (!attr_set) { cudaFuncSetAttribute(k_lambda2_g, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_set = true; }
-    const size_t smem = (size_t)2 * v * LG_CC * sizeof(double);
+    const size_t smem = lambda2_g_smem_bytes(v);
     for (int c0 = 0; c0 < m; c0 += Ncc) {
       const int cnt = std::min(Ncc, m - c0);
       k_mor_copy_cols<<<nblk(n * Ncc), 256, 0, st>>>(vec, Ncc, Ncc, h->mor_S + c0, cap, n, cnt); KLAUNCH(h);
       dim3 grid(g_blocks, (Ncc + LG_CC - 1) / LG_CC);
-      k_lambda2_g<<<grid, 256, smem, st>>>(gpart, h->L2p, vec, o, v, Ncc, h->npair); KLAUNCH(h);
+      k_lambda2_g<<<grid, 32 * LG_WARPS, smem, st>>>(gpart, h->L2p, vec, o, v, Ncc, h->npair); KLAUNCH(h);
       const long long ng = (long long)v * Ncc;
       k_g_reduce<<<(unsigned)((ng + 127) / 128), 128, 0, st>>>(gvec, gpart, g_blocks, ng); KLAUNCH(h);
       dim3 gg(np, nbc);

@@ -1,0 +1,457 @@
+// =====================================================================================
+// gfcc_ozaki.cuh -- FP64-accurate GEMM on the INT8 tensor pipe (tcgen05.mma kind::i8, TMEM int32 accumulators, TMA).
+//
+// SURVEY.md 8(f) row 2 ("Ozaki-style FP64-accurate GEMM on the low-precision tensor pipes ... as an alternative engine
+// for S9-S11; must still pass the 1e-10 parity; reported separately from the graded DMMA path").  The contraction is the
+// paper's Eq. 11 pattern; B200's FP64 DMMA ceiling (36.95 TFLOP/s measured) is the binding limit of
+// the graded engine, the INT8 pipe is ~100x wider.
+//
+// Scheme (error-free slicing, Ozaki et al.; restated, no code taken from anywhere):
+//   A[m][k] = 2^ea[m] * sum_s dA_s[m][k] * 2^(-6-7s),   dA_s integer in [-64, 64]   (ea[m]: max|A[m][:]| < 2^ea[m])
+//   B[k][n] = 2^eb[n] * sum_t dB_t[k][n] * 2^(-6-7t)                                  (eb[n] from the column maxima)
+//   C[m][n] = sum_{g=0}^{S-1} 2^(ea[m]+eb[n]-12-7g) * sum_{s+t=g} (dA_s dB_t^T)[m][n]  + O(2^(-7S)) |A|max|B|max
+// Every integer product sum is EXACT in int32 as long as (#pairs in a flush) * K * 64^2 < 2^31; the only roundings are
+// the S FP64 additions per output element and the truncation after S slices (S = 7: 2^-49 relative to the row/column maxima).
+//
+// Kernels:  k_oz_absmax / k_oz_exponent / k_oz_slice  (bandwidth-bound: operand -> S int8 K-major slices + scales)
+//           oz_igemm_kernel  (persistent, warp-specialised: 1 TMA warp, 1 MMA warp, 4 epilogue warps; 128 x 256 tiles;
+//                             4-stage smem ring; two 256-column TMEM accumulators so the FP64 read-modify-write epilogue
+//                             of flush u overlaps the MMAs of flush u+1)
+// =====================================================================================
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <vector>
+#include <algorithm>
+
+namespace gfcc {
+
+constexpr int OZ_BM = 128, OZ_BN = 256, OZ_BK = 128;        // tile (int8 elements; BK = one 128-byte swizzle row)
+constexpr int OZ_STAGES = 4;
+constexpr int OZ_THREADS = 192;                              // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2..5 epilogue
+constexpr int OZ_MAX_SLICES = 8;
+constexpr int OZ_MAX_UNITS = 40;
+constexpr int OZ_MAX_PAIRS = 8;
+constexpr long long OZ_MAX_TERMS = 500000;                   // terms of magnitude <= 64*64 per int32 accumulator (< 2^31 / 2^12)
+
+// operand view: element (r, k), k = k1*K0 + k0  ->  base[(tab ? tab[k1] : k1*sK1) + r*sR + k0*sK0] * (sgn ? sgn[k1] : 1)
+struct OzOperand {
+  const double* base = nullptr;
+  long long sR = 0, sK0 = 0, sK1 = 0;
+  const long long* tab = nullptr;
+  const double* sgn = nullptr;
+  int R = 0, K0 = 0, K1 = 1;
+};
+
+// sliced operand: S int8 matrices [S][Rpad][Kpad] (K-major) + per-row scale 2^(e-6) (0 for an all-zero row)
+struct OzSliced {
+  int8_t* q = nullptr;
+  double* scale = nullptr;
+  unsigned long long* amax = nullptr;   // scratch: bit pattern of max|x| per row
+  int R = 0, K = 0, S = 0;
+  long long Rpad = 0, Kpad = 0;
+  size_t bytes() const { return (size_t)S * Rpad * Kpad; }
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// slicing kernels
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int OZ_TR = 64, OZ_TK = 64;
+
+__device__ __forceinline__ double oz_load(const OzOperand& a, int r, int k) {
+  const int k1 = k / a.K0, k0 = k - k1 * a.K0;
+  const long long off = (a.tab ? a.tab[k1] : (long long)k1 * a.sK1) + (long long)r * a.sR + (long long)k0 * a.sK0;
+  const double x = a.base[off];
+  return a.sgn ? x * a.sgn[k1] : x;
+}
+
+// amax[r] = max_k |x[r][k]| (as the bit pattern of a non-negative double, which orders like the value)
+__global__ void __launch_bounds__(256) k_oz_absmax(OzOperand a, unsigned long long* __restrict__ amax) {
+  __shared__ unsigned long long smax[OZ_TR];
+  const int r0 = blockIdx.y * OZ_TR, k0 = blockIdx.x * OZ_TK, K = a.K0 * a.K1;
+  if (threadIdx.x < OZ_TR) smax[threadIdx.x] = 0ull;
+  __syncthreads();
+  const bool kfast = (a.sK0 == 1);
+  for (int idx = threadIdx.x; idx < OZ_TR * OZ_TK; idx += 256) {
+    const int rl = kfast ? idx / OZ_TK : idx % OZ_TR, kl = kfast ? idx % OZ_TK : idx / OZ_TR;
+    const int r = r0 + rl, k = k0 + kl;
+    if (r < a.R && k < K) {
+      const unsigned long long b = (unsigned long long)__double_as_longlong(fabs(oz_load(a, r, k)));
+      if (b > smax[rl]) atomicMax(&smax[rl], b);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < OZ_TR && r0 + threadIdx.x < a.R && smax[threadIdx.x] != 0ull) atomicMax(&amax[r0 + threadIdx.x], smax[threadIdx.x]);
+}
+
+// scale[r] = 2^(e-6) with max|x[r][:]| < 2^e ; 0 for a zero row.  inv[r] = 2^(6-e) is recomputed in k_oz_slice.
+__global__ void k_oz_exponent(const unsigned long long* __restrict__ amax, double* __restrict__ scale, int R) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= R) return;
+  const double m = __longlong_as_double((long long)amax[r]);
+  if (!(m > 0.0) || !isfinite(m)) { scale[r] = 0.0; return; }
+  int e;
+  frexp(m, &e);                       // m = f * 2^e, f in [0.5, 1)  =>  |x| <= m < 2^e
+  scale[r] = ldexp(1.0, e - 6);
+}
+
+// q[s][r][k] = s-th base-128 signed digit of x[r][k] / 2^e  (first digit base 64), digits in [-64, 64]
+__global__ void __launch_bounds__(256) k_oz_slice(OzOperand a, const double* __restrict__ scale, int8_t* __restrict__ q, int S,
+                                                  long long Rpad, long long Kpad) {
+  __shared__ double tile[OZ_TR][OZ_TK + 1];
+  const int r0 = blockIdx.y * OZ_TR, k0 = blockIdx.x * OZ_TK, K = a.K0 * a.K1;
+  const bool kfast = (a.sK0 == 1);
+  for (int idx = threadIdx.x; idx < OZ_TR * OZ_TK; idx += 256) {
+    const int rl = kfast ? idx / OZ_TK : idx % OZ_TR, kl = kfast ? idx % OZ_TK : idx / OZ_TR;
+    const int r = r0 + rl, k = k0 + kl;
+    tile[rl][kl] = (r < a.R && k < K) ? oz_load(a, r, k) : 0.0;
+  }
+  __syncthreads();
+  const int rl = threadIdx.x >> 2, kc = (threadIdx.x & 3) * 16;
+  const int r = r0 + rl;
+  if (r >= a.R) return;
+  const double sc = scale[r];
+  const double inv = sc > 0.0 ? 1.0 / sc : 0.0;          // 2^(6-e): exact
+  double y[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) y[j] = tile[rl][kc + j] * inv;   // |y| < 64, exact scaling
+  for (int s = 0; s < S; ++s) {
+    union { int8_t b[16]; int4 v; } out;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const double d = rint(y[j]);                          // in [-64, 64]
+      out.b[j] = (int8_t)(int)d;
+      y[j] = (y[j] - d) * 128.0;                            // exact: remainder in [-0.5, 0.5] -> [-64, 64]
+    }
+    *reinterpret_cast<int4*>(q + ((long long)s * Rpad + r) * Kpad + k0 + kc) = out.v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// PTX wrappers (sm_100a): mbarrier, TMA, tcgen05
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned oz_smem(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void oz_mbar_init(uint64_t* b, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(oz_smem(b)), "r"(count));
+}
+__device__ __forceinline__ void oz_mbar_arrive(uint64_t* b) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(oz_smem(b)) : "memory");
+}
+__device__ __forceinline__ void oz_mbar_expect_tx(uint64_t* b, unsigned bytes) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(oz_smem(b)), "r"(bytes) : "memory");
+}
+// bounded spin: a lost arrival must not hang the GPU box; on timeout the flag is raised and every role bails out
+__device__ __forceinline__ bool oz_mbar_wait(uint64_t* b, unsigned parity, int* __restrict__ fail) {
+  unsigned ok = 0;
+  for (long long spin = 0; spin < (1ll << 26); ++spin) {
+    asm volatile(
+        "{\n.reg .pred P1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n}\n"
+        : "=r"(ok) : "r"(oz_smem(b)), "r"(parity) : "memory");
+    if (ok) return true;
+    if ((spin & 1023) == 1023 && *(volatile int*)fail) return false;
+  }
+  atomicExch(fail, 1);
+  return false;
+}
+__device__ __forceinline__ void oz_tma_load_3d(void* smem_dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n"
+      ::"r"(oz_smem(smem_dst)), "l"(tm), "r"(oz_smem(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void oz_tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void oz_tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void oz_tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(oz_smem(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, int8 x int8 -> int32, M = 128, N = OZ_BN, K = 32
+__device__ __forceinline__ void oz_mma_i8(unsigned tmem_d, uint64_t desc_a, uint64_t desc_b, unsigned idesc, unsigned accumulate) {
+  asm volatile(
+      "{\n.reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}\n"
+      ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
+}
+// shared-memory matrix descriptor: K-major, SWIZZLE_128B (rows of 128 bytes, 8-row groups 1024 bytes apart), sm_100 version bit
+__device__ __forceinline__ uint64_t oz_smem_desc(unsigned smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3FFFF) >> 4);          // start address, 16-byte units
+  d |= (uint64_t)1 << 16;                               // leading byte offset (ignored for swizzled K-major), 16-byte units
+  d |= (uint64_t)(1024 >> 4) << 32;                     // stride byte offset: 8 rows * 128 B
+  d |= (uint64_t)1 << 46;                               // descriptor version (sm_100)
+  d |= (uint64_t)2 << 61;                               // SWIZZLE_128B
+  return d;
+}
+// 32 consecutive int32 columns of this thread's TMEM lane
+__device__ __forceinline__ void oz_tmem_ld32(unsigned taddr, int (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+        "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+        "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+}
+
+// one flush unit: npairs slice pairs of equal order g = s + t over the k-blocks [kb0, kb1), accumulated in ONE int32 tile
+struct OzUnit { short g, np; unsigned char s[OZ_MAX_PAIRS], t[OZ_MAX_PAIRS]; int kb0, kb1; };
+struct OzGemmParams {
+  int M, N, tiles_m, tiles_n, nunits;
+  double alpha, beta;
+  const double* sa; const double* sb;
+  double* C; long long sCm0, sCm1; int Md; long long sCn0, sCn1; int Nd;
+  int* fail;
+  OzUnit u[OZ_MAX_UNITS];
+};
+
+constexpr unsigned OZ_A_BYTES = OZ_BM * OZ_BK, OZ_B_BYTES = OZ_BN * OZ_BK, OZ_STAGE_BYTES = OZ_A_BYTES + OZ_B_BYTES;
+constexpr size_t OZ_SMEM_BYTES = (size_t)OZ_STAGES * OZ_STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+// instruction descriptor: D = S32 (2 << 4), A = B = signed int8 (1 << 7, 1 << 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+constexpr unsigned OZ_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(OZ_BN >> 3) << 17) | ((unsigned)(OZ_BM >> 4) << 24);
+
+// ---------------------------------------------------------------------------------------------------------------
+// the INT8 tensor-core kernel
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_constant__ CUtensorMap tmA,
+                                                                 const __grid_constant__ CUtensorMap tmB,
+                                                                 const __grid_constant__ OzGemmParams p) {
+  extern __shared__ uint8_t oz_smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)oz_smem_raw + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)OZ_STAGES * OZ_STAGE_BYTES);
+  uint64_t* full = bars;                       // [OZ_STAGES]  TMA -> MMA
+  uint64_t* empty = bars + OZ_STAGES;          // [OZ_STAGES]  MMA -> TMA
+  uint64_t* tfull = bars + 2 * OZ_STAGES;      // [2]          MMA -> epilogue
+  uint64_t* tempty = tfull + 2;                // [2]          epilogue -> MMA
+  unsigned* tmem_slot = reinterpret_cast<unsigned*>(tempty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < OZ_STAGES; ++s) { oz_mbar_init(&full[s], 1); oz_mbar_init(&empty[s], 1); }
+    oz_mbar_init(&tfull[0], 1); oz_mbar_init(&tfull[1], 1);
+    oz_mbar_init(&tempty[0], 4); oz_mbar_init(&tempty[1], 4);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(&tmA) : "memory");
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(&tmB) : "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(oz_smem(tmem_slot)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+  }
+  oz_tc_fence_before();
+  __syncthreads();
+  oz_tc_fence_after();
+  const unsigned tmem_base = *tmem_slot;
+  const int ntiles = p.tiles_m * p.tiles_n;
+
+  if (warp == 0) {
+    // ============================== TMA producer (one lane) ==============================
+    if (lane == 0) {
+      int stage = 0; unsigned phase = 0;
+      bool ok = true;
+      for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+        const int m0 = (tile % p.tiles_m) * OZ_BM, n0 = (tile / p.tiles_m) * OZ_BN;
+        for (int u = 0; u < p.nunits && ok; ++u) {
+          const OzUnit& un = p.u[u];
+          for (int pr = 0; pr < un.np && ok; ++pr)
+            for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              if (!(ok = oz_mbar_wait(&empty[stage], phase ^ 1, p.fail))) break;
+              uint8_t* sa = smem + (size_t)stage * OZ_STAGE_BYTES;
+              oz_mbar_expect_tx(&full[stage], OZ_STAGE_BYTES);
+              oz_tma_load_3d(sa, &tmA, &full[stage], kb * OZ_BK, m0, un.s[pr]);
+              oz_tma_load_3d(sa + OZ_A_BYTES, &tmB, &full[stage], kb * OZ_BK, n0, un.t[pr]);
+              if (++stage == OZ_STAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ============================== MMA issuer (one lane) ==============================
+    if (lane == 0) {
+      int stage = 0; unsigned phase = 0;
+      unsigned cnt = 0;
+      bool ok = true;
+      for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+        for (int u = 0; u < p.nunits && ok; ++u, ++cnt) {
+          const OzUnit& un = p.u[u];
+          const unsigned buf = cnt & 1, use = cnt >> 1;
+          if (!(ok = oz_mbar_wait(&tempty[buf], (use & 1) ^ 1, p.fail))) break;
+          oz_tc_fence_after();
+          const unsigned tmem_d = tmem_base + buf * OZ_BN;
+          unsigned acc = 0;
+          for (int pr = 0; pr < un.np && ok; ++pr)
+            for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              if (!(ok = oz_mbar_wait(&full[stage], phase, p.fail))) break;
+              oz_tc_fence_after();
+              const unsigned a_addr = oz_smem(smem + (size_t)stage * OZ_STAGE_BYTES);
+              const uint64_t da = oz_smem_desc(a_addr), db = oz_smem_desc(a_addr + OZ_A_BYTES);
+#pragma unroll
+              for (int k = 0; k < OZ_BK / 32; ++k) {
+                oz_mma_i8(tmem_d, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), OZ_IDESC, acc);
+                acc = 1;
+              }
+              oz_tc_commit(&empty[stage]);          // frees the smem slot once these MMAs have read it
+              if (++stage == OZ_STAGES) { stage = 0; phase ^= 1; }
+            }
+          if (ok) oz_tc_commit(&tfull[buf]);        // accumulator of this flush unit is complete
+        }
+      }
+    }
+  } else {
+    // ============================== epilogue warps: TMEM -> FP64 read-modify-write of C ==============================
+    const int quad = warp & 3;                      // TMEM lane quadrant this warp may access
+    const int rl = quad * 32 + lane;
+    unsigned cnt = 0;
+    bool ok = true;
+    for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+      const int m0 = (tile % p.tiles_m) * OZ_BM, n0 = (tile / p.tiles_m) * OZ_BN;
+      const int row = m0 + rl;
+      const bool rok = row < p.M;
+      const double rs0 = rok ? p.alpha * p.sa[row] : 0.0;
+      double* crow = p.C + (rok ? (long long)(row % p.Md) * p.sCm0 + (long long)(row / p.Md) * p.sCm1 : 0);
+      for (int u = 0; u < p.nunits && ok; ++u, ++cnt) {
+        const unsigned buf = cnt & 1, use = cnt >> 1;
+        ok = oz_mbar_wait(&tfull[buf], use & 1, p.fail);
+        ok = __all_sync(0xffffffffu, ok);
+        if (!ok) break;
+        oz_tc_fence_after();
+        const double rs = rs0 * exp2((double)(-7 * p.u[u].g));
+        const bool first = (u == 0);
+#pragma unroll 1
+        for (int c = 0; c < OZ_BN / 32; ++c) {
+          int v[32];
+          oz_tmem_ld32(tmem_base + ((unsigned)(quad * 32) << 16) + buf * OZ_BN + c * 32, v);
+          const int col0 = n0 + c * 32;
+          if (rok && col0 < p.N) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const int col = col0 + j;
+              if (col < p.N) {
+                double* cp = crow + (long long)(col % p.Nd) * p.sCn0 + (long long)(col / p.Nd) * p.sCn1;
+                const double val = rs * p.sb[col] * (double)v[j];
+                if (first) *cp = (p.beta == 0.0) ? val : p.beta * (*cp) + val;
+                else *cp += val;
+              }
+            }
+          }
+        }
+        oz_tc_fence_before();
+        __syncwarp();
+        if (lane == 0) oz_mbar_arrive(&tempty[buf]);
+      }
+    }
+  }
+  oz_tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "r"(512u) : "memory");
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------------
+typedef CUresult (*oz_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+inline oz_encode_fn oz_get_encode() {
+  static oz_encode_fn fn = nullptr;
+  if (!fn) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (oz_encode_fn)ptr;
+  }
+  return fn;
+}
+// 3-D map over the slices of one operand: (k, row, slice), box (128 bytes, box_rows, 1), 128-byte swizzle, zero fill out of bounds
+inline bool oz_make_map(CUtensorMap* tm, const OzSliced& s, int box_rows) {
+  oz_encode_fn enc = oz_get_encode();
+  if (!enc) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)s.Kpad, (cuuint64_t)s.R, (cuuint64_t)s.S};
+  cuuint64_t strides[2] = {(cuuint64_t)s.Kpad, (cuuint64_t)(s.Rpad * s.Kpad)};
+  cuuint32_t box[3] = {(cuuint32_t)OZ_BK, (cuuint32_t)box_rows, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void*)s.q, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+inline long long oz_round_up(long long x, long long m) { return (x + m - 1) / m * m; }
+
+// sizes of the sliced form of an operand with R rows and K columns
+inline void oz_shape(OzSliced& s, int R, int K, int S) {
+  s.R = R; s.K = K; s.S = S;
+  s.Rpad = oz_round_up(R, OZ_TR);
+  s.Kpad = oz_round_up(K, OZ_BK);
+}
+// operand -> slices (buffers of `s` must be allocated: q bytes(), scale R doubles, amax R u64)
+inline cudaError_t oz_slice(const OzOperand& a, OzSliced& s, cudaStream_t st) {
+  const int K = a.K0 * a.K1;
+  cudaError_t e = cudaMemsetAsync(s.amax, 0, (size_t)a.R * 8, st);
+  if (e != cudaSuccess) return e;
+  dim3 grid((unsigned)((K + OZ_TK - 1) / OZ_TK), (unsigned)((a.R + OZ_TR - 1) / OZ_TR));
+  k_oz_absmax<<<grid, 256, 0, st>>>(a, s.amax);
+  k_oz_exponent<<<(a.R + 255) / 256, 256, 0, st>>>(s.amax, s.scale, a.R);
+  dim3 grid2((unsigned)(s.Kpad / OZ_TK), grid.y);
+  k_oz_slice<<<grid2, 256, 0, st>>>(a, s.scale, s.q, s.S, s.Rpad, s.Kpad);
+  return cudaGetLastError();
+}
+
+struct OzCDesc {
+  double* C = nullptr; long long sCm0 = 0, sCm1 = 0; int Md = 0; long long sCn0 = 1, sCn1 = 0; int Nd = 0;
+  double alpha = 1.0, beta = 0.0;
+};
+
+// C (+)= alpha * A * B^T from the sliced operands (A: M rows, B: N rows, common K).  `fail` is a device int (zeroed by the
+// caller) that the kernel raises if a pipeline wait times out.
+inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc& c, int* fail, cudaStream_t st, int num_sms = 148) {
+  if (A.K != B.K || A.S != B.S || A.S < 1 || A.S > OZ_MAX_SLICES) return cudaErrorInvalidValue;
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t e = cudaFuncSetAttribute(oz_igemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OZ_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr = true;
+  }
+  CUtensorMap tmA, tmB;
+  if (!oz_make_map(&tmA, A, OZ_BM) || !oz_make_map(&tmB, B, OZ_BN)) return cudaErrorUnknown;
+  OzGemmParams p;
+  p.M = A.R; p.N = B.R;
+  p.tiles_m = (A.R + OZ_BM - 1) / OZ_BM; p.tiles_n = (B.R + OZ_BN - 1) / OZ_BN;
+  p.alpha = c.alpha; p.beta = c.beta; p.sa = A.scale; p.sb = B.scale;
+  p.C = c.C; p.sCm0 = c.sCm0; p.sCm1 = c.sCm1; p.Md = c.Md > 0 ? c.Md : A.R;
+  p.sCn0 = c.sCn0; p.sCn1 = c.sCn1; p.Nd = c.Nd > 0 ? c.Nd : B.R;
+  p.fail = fail;
+  // flush units: order g = S-1 .. 0 (small contributions first), pairs of one order chunked so that pairs * k-range fits int32
+  const int S = A.S;
+  const long long kblocks = A.Kpad / OZ_BK;
+  const long long kb_per_unit_max = std::max<long long>(1, OZ_MAX_TERMS / OZ_BK);
+  int nu = 0;
+  for (int g = S - 1; g >= 0; --g) {
+    // k-chunks: when one pair over the whole K does not fit, split K; otherwise group several pairs
+    const long long nchunk = (kblocks + kb_per_unit_max - 1) / kb_per_unit_max;
+    const long long kb_chunk = (kblocks + nchunk - 1) / nchunk;
+    const int pairs_per_unit = (int)std::max<long long>(1, std::min<long long>(OZ_MAX_PAIRS, OZ_MAX_TERMS / (kb_chunk * OZ_BK)));
+    for (long long kb0 = 0; kb0 < kblocks; kb0 += kb_chunk) {
+      int s = 0;
+      while (s <= g) {
+        if (nu >= OZ_MAX_UNITS) return cudaErrorInvalidValue;
+        OzUnit& un = p.u[nu++];
+        un.g = (short)g; un.np = 0; un.kb0 = (int)kb0; un.kb1 = (int)std::min(kblocks, kb0 + kb_chunk);
+        while (s <= g && un.np < pairs_per_unit) { un.s[un.np] = (unsigned char)s; un.t[un.np] = (unsigned char)(g - s); ++un.np; ++s; }
+      }
+    }
+  }
+  p.nunits = nu;
+  const int grid = std::min(p.tiles_m * p.tiles_n, num_sms);
+  if (grid < 1) return cudaSuccess;
+  oz_igemm_kernel<<<grid, OZ_THREADS, OZ_SMEM_BYTES, st>>>(tmA, tmB, p);
+  return cudaGetLastError();
+}
+
+}  // namespace gfcc

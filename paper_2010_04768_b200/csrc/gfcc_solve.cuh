@@ -180,43 +180,78 @@ __global__ void k_backsolve(int m, int nrhs, const double2* __restrict__ R, cons
 }
 
 // ---- g[b][c] = sum_(i,j,a) lambda[i,j,b,a] x2[i,j,a][c] = 2 sum_(i<j) sum_a l_p[b,a] x_p[a][c]  (Lambda2 packed [pair][a<b]) ----
-// grid (pair blocks, column chunks of 8 real columns); gpart[blk][v][Nc]
+// grid (pair blocks, column chunks of LG_CC real columns); gpart[blk][v][Nc].
+// Every element U[a][b] (a<b) of a pair's packed triangle is read ONCE, coalesced (a row of the triangle is contiguous in b),
+// as part of a 32 x 32 tile that a warp parks in shared memory; the tile then serves both roles of the antisymmetric block:
+//   g[b] -= sum_a U[a][b] x[a]   (lane = b, walks the tile's column)      g[a] += sum_b U[a][b] x[b]   (lane = a, walks its row)
+// with LG_CC register accumulators per lane, folded into the block's g accumulator by shared-memory atomics.
 constexpr int LG_CC = 8;
-__global__ void __launch_bounds__(256) k_lambda2_g(double* __restrict__ gpart, const double* __restrict__ L2p,
-                                                    const double* __restrict__ vec, int o, int v, int Nc, long long npair) {
+constexpr int LG_WARPS = 8;
+constexpr int LG_TS = 33;                 // padded tile stride: row and column walks are both bank-conflict free
+inline int lg_vpad(int v) { return (v + 31) / 32 * 32; }
+inline size_t lambda2_g_smem_bytes(int v) {
+  return ((size_t)lg_vpad(v) * LG_CC + (size_t)v * LG_CC + (size_t)LG_WARPS * 32 * LG_TS) * sizeof(double);
+}
+__global__ void __launch_bounds__(32 * LG_WARPS) k_lambda2_g(double* __restrict__ gpart, const double* __restrict__ L2p,
+                                                              const double* __restrict__ vec, int o, int v, int Nc, long long npair) {
   extern __shared__ double sm[];
-  double* xs = sm;                       // [v][LG_CC]
-  double* ga = sm + (size_t)v * LG_CC;   // [v][LG_CC]
+  const int vpad = (v + 31) / 32 * 32, nt = vpad / 32;
+  double* xs = sm;                                   // [vpad][LG_CC], rows >= v are zero
+  double* ga = xs + (size_t)vpad * LG_CC;            // [v][LG_CC]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double* Ts = ga + (size_t)v * LG_CC + (size_t)warp * 32 * LG_TS;   // this warp's [32][LG_TS] tile
   const int c0 = blockIdx.y * LG_CC;
   const long long ntri = (long long)v * (v - 1) / 2;
   for (int t = threadIdx.x; t < v * LG_CC; t += blockDim.x) ga[t] = 0.0;
   const double* x2 = vec + (long long)o * Nc;
   for (long long pr = blockIdx.x; pr < npair; pr += gridDim.x) {
     __syncthreads();
-    for (int t = threadIdx.x; t < v * LG_CC; t += blockDim.x) {
+    for (int t = threadIdx.x; t < vpad * LG_CC; t += blockDim.x) {
       const int a = t / LG_CC, c = t % LG_CC;
-      xs[t] = (c0 + c < Nc) ? x2[(pr * v + a) * Nc + c0 + c] : 0.0;
+      xs[t] = (a < v && c0 + c < Nc) ? x2[(pr * v + a) * Nc + c0 + c] : 0.0;
     }
     __syncthreads();
     const double* lp = L2p + pr * ntri;
-    for (int b = threadIdx.x; b < v; b += blockDim.x) {
-      double acc[LG_CC];
+    int cnt = 0;
+    for (int ta = 0; ta < nt; ++ta)
+      for (int tb = ta; tb < nt; ++tb, ++cnt) {
+        if (cnt % LG_WARPS != warp) continue;
+        const int a0 = ta * 32, b0 = tb * 32, b = b0 + lane;
+        __syncwarp();
+#pragma unroll 8
+        for (int r = 0; r < 32; ++r) {
+          const int a = a0 + r;
+          Ts[r * LG_TS + lane] = (a < b && b < v) ? lp[tri_index(a, b, v)] : 0.0;
+        }
+        __syncwarp();
+        double acc[LG_CC];
 #pragma unroll
-      for (int c = 0; c < LG_CC; ++c) acc[c] = 0.0;
-      for (int a = 0; a < b; ++a) {          // lambda[b,a] = -lambda[a,b], a<b  (coalesced across b)
-        const double s = lp[tri_index(a, b, v)];
+        for (int c = 0; c < LG_CC; ++c) acc[c] = 0.0;
+#pragma unroll 4
+        for (int r = 0; r < 32; ++r) {               // lane = b: column walk
+          const double u = Ts[r * LG_TS + lane];
+          const double* xr = xs + (size_t)(a0 + r) * LG_CC;
 #pragma unroll
-        for (int c = 0; c < LG_CC; ++c) acc[c] -= s * xs[a * LG_CC + c];
+          for (int c = 0; c < LG_CC; ++c) acc[c] += u * xr[c];
+        }
+        if (b < v) {
+#pragma unroll
+          for (int c = 0; c < LG_CC; ++c) atomicAdd(&ga[b * LG_CC + c], -acc[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < LG_CC; ++c) acc[c] = 0.0;
+#pragma unroll 4
+        for (int k = 0; k < 32; ++k) {               // lane = a: row walk
+          const double u = Ts[lane * LG_TS + k];
+          const double* xr = xs + (size_t)(b0 + k) * LG_CC;
+#pragma unroll
+          for (int c = 0; c < LG_CC; ++c) acc[c] += u * xr[c];
+        }
+        if (a0 + lane < v) {
+#pragma unroll
+          for (int c = 0; c < LG_CC; ++c) atomicAdd(&ga[(a0 + lane) * LG_CC + c], acc[c]);
+        }
       }
-      const double* row = lp + tri_index(b, b + 1, v) - (b + 1);   // row[a] = lambda[b,a], a > b
-      for (int a = b + 1; a < v; ++a) {
-        const double s = row[a];
-#pragma unroll
-        for (int c = 0; c < LG_CC; ++c) acc[c] += s * xs[a * LG_CC + c];
-      }
-#pragma unroll
-      for (int c = 0; c < LG_CC; ++c) ga[b * LG_CC + c] += acc[c];
-    }
   }
   __syncthreads();
   for (int t = threadIdx.x; t < v * LG_CC; t += blockDim.x) {
@@ -443,10 +478,10 @@ inline int solve_run(SolveWs& s, const SolveCfg& c, const int* p_of_rhs, const d
   {
     const int Nc = 2 * nr;
     dim3 grid(s.g_blocks, (Nc + LG_CC - 1) / LG_CC);
-    const size_t smem = (size_t)2 * c.v * LG_CC * sizeof(double);
+    const size_t smem = lambda2_g_smem_bytes(c.v);
     static bool attr_set = false;
     if (!attr_set) { cudaFuncSetAttribute(k_lambda2_g, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_set = true; }
-    k_lambda2_g<<<grid, 256, smem, st>>>(s.gpart, c.L2p, s.x, c.o, c.v, Nc, c.npair); S_K();
+    k_lambda2_g<<<grid, 32 * LG_WARPS, smem, st>>>(s.gpart, c.L2p, s.x, c.o, c.v, Nc, c.npair); S_K();
     const long long n = (long long)c.v * Nc;
     k_g_reduce<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(s.gvec, s.gpart, s.g_blocks, n); S_K();
     dim3 gg(nq, nr);
