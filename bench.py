@@ -49,6 +49,10 @@ def parse():
                     help="(internal) child process of the default run: time the oracle sample, print its JSON, exit")
     ap.add_argument("--cpu-baseline-serial", action="store_true",
                     help="time the oracle AFTER the GPU part on all host cores instead of beside it (doubles the run time at config 4)")
+    ap.add_argument("--engine", default="dmma", choices=["dmma", "ozaki"],
+                    help="dmma: FP64 tensor-core engine (graded default); ozaki: S8-S11 on the INT8 tensor pipe with FP64 accuracy "
+                         "(SURVEY.md 8f row 2, reported separately)")
+    ap.add_argument("--slices", type=int, default=7, help="digit slices of the ozaki engine (7: ~1e-13, 6: ~1e-11 per GEMM)")
     ap.add_argument("--overlap", type=int, default=-1, help="1: run independent sigma panel chains on side streams (default: library default)")
     return ap.parse_args()
 
@@ -284,6 +288,10 @@ def main():
     g.gfcc_set_option(h, "max_batch", nrhs)
     if args.overlap >= 0:
         g.gfcc_set_option(h, "overlap", args.overlap)
+    if args.engine == "ozaki":
+        g.gfcc_set_option(h, "ozaki_slices", args.slices)
+        g.gfcc_set_option(h, "engine", 1)
+        g.gfcc_set_option(h, "panel_bytes", 4.2e9)
 
     # rank r solves its own slice of the omega sweep (independent (p,omega) tasks; weak scaling)
     omegas = sharding.weak_scaling_grid(c["wlo"], c["whi"], c["nw"], max(world, 1), rank)
@@ -332,6 +340,7 @@ def main():
     gemm_ms = g.gfcc_get_stat(h, "gemm_time_ms")
     gemm_flops = g.gfcc_get_stat(h, "gemm_flops_timed")
     gemm_n = g.gfcc_get_stat(h, "gemm_launches_timed")
+    oz_ms, oz_ops, oz_fl, oz_n = (g.gfcc_get_stat(h, k) for k in ("oz_time_ms", "oz_ops_timed", "oz_flops_timed", "oz_launches_timed"))
     g.gfcc_set_option(h, "profile_gemm", 0)
     ms_total = sharding.max_over_ranks(ms_total, world, dist, "cuda")
     ms_step = ms_total / args.steps
@@ -347,7 +356,10 @@ def main():
                    "flop_model": "executed Cholesky-route model, SURVEY.md 8(d): real x complex = 2 real products, pair-packed o^4 term",
                    "flops_per_sigma_application": flops_sigma, "sigma_applications_per_step": apps_per_step,
                    "gmres_m_used": g.gfcc_get_stat(h, "gmres_m_used"), "overlap": int(overlap_on),
-                   "gemm_engine": os.environ.get("GFCC_GEMM_ENGINE", "ws"), "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
+                   "gemm_engine": (os.environ.get("GFCC_GEMM_ENGINE", "ws") if args.engine == "dmma" else
+                                   f"ozaki_int8 x{args.slices} slices for S8-S11 (tcgen05.mma kind::i8, exact int32 accumulation, FP64-accurate; "
+                                   "NOT the graded FP64 DMMA engine), rest on the DMMA engine"),
+                   "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
         "solves_per_s": solves_per_s, "solves_note": f"(p,omega) right-hand sides advanced by {kfix} GMRES steps per second x nrhs",
         "pct_fp64_peak_measured": 100.0 * value / world / FP64_DMMA_PEAK_TFLOPS,
         "create_s": create_s, "create_tflops": flops_create / create_s / 1e12, "inputs_s": t_inputs,
@@ -373,6 +385,20 @@ def main():
                         "step), whose algorithmic bytes (A + B + C once) are 8.2e9; DRAM is 4.9 % busy in that launch (tensor-bound, 91.7 % DMMA "
                         "pipe), L2 hit 80 %; null for configs without a capture",
     }
+
+    if args.engine == "ozaki" and oz_ms > 0:
+        i8_peak = (mp["bf16_tflops_sustained"] * 2.0) if mp else 2.0 * 1365.7
+        r = line["roofline"]
+        line["roofline_dmma_part"] = {k: r[k] for k in ("achieved", "launches", "share_of_step")}
+        line["roofline"] = {
+            "kernel": "gfcc::oz_igemm_kernel (INT8 tcgen05 launches of the timed region: S8-S11)", "bound": "tensor",
+            "achieved": oz_ops / (oz_ms * 1e-3) / 1e12, "peak": i8_peak, "unit": "TFLOP/s", "frac": oz_ops / (oz_ms * 1e-3) / 1e12 / i8_peak,
+            "peak_source": "int8 dense = sustained bf16 of MEASURED_PEAKS.json x nominal ratio 4.5/2.25 (no measured int8 entry); unit is int8 TOP/s",
+            "launches": int(oz_n), "avg_launch_ms": oz_ms / max(oz_n, 1), "share_of_step": oz_ms / ms_prof if ms_prof > 0 else None,
+            "algorithmic_flops": oz_fl, "fp64_equivalent_tflops": oz_fl / (oz_ms * 1e-3) / 1e12,
+            "int8_ops": oz_ops, "traffic": None,
+            "note": "int8 ops = 2MNK x S(S+1)/2 digit-matrix products; fp64_equivalent = 2MNK / time"}
+        line["pct_fp64_peak_note"] = "above 100 % by construction: the work runs on the INT8 pipe, FP64 DMMA peak is only the yardstick"
 
     # ---- end to end through the C ABI with HOST buffers: one batched sigma application, copies inside the call ----
     if not args.no_e2e and rank == 0:

@@ -146,6 +146,18 @@ int gfcc_destroy(gfcc_handle h);
 int gfcc_dgemm(void* cuda_stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
                const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn);
 
+/* FP64-accurate GEMM on the INT8 tensor pipe ("Ozaki-style FP64-accurate GEMM on the low-precision
+ * tensor pipes"; the contraction is Eq. 11's pattern).  Same operand conventions as gfcc_dgemm.
+ * A's rows and B's columns are scaled by powers of two and cut into `nslices` (1..8) signed 7-bit digit matrices
+ * (error-free, int8, K-major); all digit-matrix products of order s+t < nslices run on tcgen05.mma kind::i8 with exact
+ * int32 accumulation in TMEM and are added into C in FP64.  Truncation error <= ~2^(-7*nslices) * max|A row| * max|B col|
+ * per term (nslices = 7: 2^-49).  Synchronous; scratch is allocated and freed inside.  ms_slice / ms_gemm [host,
+ * nullable] receive the CUDA-event times of the slicing passes and of the tensor-core kernel.
+ * Returns GFCC_EINVAL (bad sizes/strides), GFCC_ENOMEM, GFCC_ECUDA (launch failure or pipeline time-out).            */
+int gfcc_dgemm_ozaki(void* cuda_stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
+                     const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn,
+                     int nslices, double* ms_slice, double* ms_gemm);
+
 /* Roofline denominator of the sigma contractions: measured issue-rate ceiling of the FP64 tensor-pipe instruction
  * the GEMM engine is built on (mma.sync m8n8k4 f64 = SASS DMMA), register-only loop on every SM, CUDA events on
  * `cuda_stream`.  iters: DMMAs per accumulator chain (>= 1; 20000 gives a ~30 ms launch); reps: timed launches

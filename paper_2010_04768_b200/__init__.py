@@ -23,7 +23,7 @@ GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 
 EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_intermediate", "gfcc_last_error",
-           "gfcc_destroy", "gfcc_dgemm", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
+           "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
            "gfcc_mor_get"]
 
 
@@ -62,6 +62,7 @@ def lib():
     L.gfcc_last_error.restype = ctypes.c_char_p
     L.gfcc_destroy.argtypes = [vp]
     L.gfcc_dgemm.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll]
+    L.gfcc_dgemm_ozaki.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll, ci, dp, dp]
     L.gfcc_probe_fp64_peak.argtypes = [vp, ci, ci, dp]
     L.gfcc_mor_reset.argtypes = [vp, ci]
     L.gfcc_mor_extend.argtypes = [vp, ci, vp, vp, cd, ip]
@@ -240,6 +241,24 @@ def gfcc_dgemm(A, B, C=None, alpha=1.0, beta=0.0, stream=0):
     if rc != GFCC_OK:
         raise GfccError(rc, "gfcc_dgemm failed")
     return C
+
+
+def gfcc_dgemm_ozaki(A, B, C=None, alpha=1.0, beta=0.0, nslices=7, stream=0, return_times=False):
+    """C = alpha * A @ B + beta * C on the INT8 tensor pipe with FP64 accuracy (error-free slicing; include/gfcc.h)."""
+    torch = _torch()
+    M, K = A.shape
+    K2, N = B.shape
+    assert K == K2
+    if C is None:
+        C = torch.zeros((M, N), dtype=torch.float64, device=A.device)
+    ms_s, ms_g = ctypes.c_double(), ctypes.c_double()
+    rc = lib().gfcc_dgemm_ozaki(ctypes.c_void_p(stream), M, N, K, float(alpha), ctypes.c_void_p(A.data_ptr()), A.stride(0),
+                                A.stride(1), ctypes.c_void_p(B.data_ptr()), B.stride(0), B.stride(1), float(beta),
+                                ctypes.c_void_p(C.data_ptr()), C.stride(0), C.stride(1), int(nslices), ctypes.byref(ms_s),
+                                ctypes.byref(ms_g))
+    if rc != GFCC_OK:
+        raise GfccError(rc, "gfcc_dgemm_ozaki failed")
+    return (C, ms_s.value, ms_g.value) if return_times else C
 
 
 def gfcc_probe_fp64_peak(iters=20000, reps=5, stream=0):

@@ -55,6 +55,13 @@ struct gfcc_ctx {
   double *vin = nullptr, *vout = nullptr;   // internal vectors for gfcc_sigma_ip
   long long part_elems = 0;
   int panel_ni = 1;
+  // ---- INT8 tensor-core (Ozaki) engine for S8-S11 (gfcc_ozaki.cuh, gfcc_ozaki_host.inl; option "engine" = 1) ----
+  int opt_engine = 0, opt_oz_slices = 7;
+  OzSliced ozLvv, ozLooT, ozLov, ozXU, ozKP;
+  int* oz_fail = nullptr;
+  bool oz_const_ready = false;
+  int oz_ws_nrhs = 0, oz_ws_ni = 0;
+  double st_oz_gemms = 0;
   // ---- options / stats ----
   double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3e9, opt_max_batch = 256, opt_overlap = 0;
   double st_iterations = 0, st_sigma_apps = 0, st_flops_sigma = 0, st_flops_create = 0, st_max_relres = 0, st_nunconv = 0;
@@ -72,6 +79,7 @@ struct gfcc_ctx {
   std::vector<cudaEvent_t> ev_pool;
   size_t ev_used = 0;
   std::vector<double> ev_flops;   // flops of the launch bracketed by events (2k, 2k+1)
+  std::vector<double> ev_ops8;    // int8 multiply-add operations x2 of that launch (0 for an FP64 DMMA launch)
 };
 
 #define CUDA_TRY(h, expr)                                                                      \
@@ -122,6 +130,7 @@ static int gemm(gfcc_ctx* h, const GemmDesc& d) {
     CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used + 1], h->cur));
     h->ev_used += 2;
     h->ev_flops.push_back(2.0 * d.M * (double)d.N * (double)d.K1 * d.K0 * d.batch);
+    h->ev_ops8.push_back(0.0);
   }
   h->st_gemm_launches += 1;
   h->st_kernel_launches += 1;
@@ -170,8 +179,11 @@ static inline unsigned nblk(long long n, int t = 256, long long cap = 148LL * 32
 // ------------------------------------------------------------------------------------------
 // workspace for a batch of nrhs right-hand sides
 // ------------------------------------------------------------------------------------------
+#include "gfcc_ozaki_host.inl"
+
 static void free_workspace(gfcc_ctx* h) {
   const int o = h->o, v = h->v;
+  oz_free_ws(h);
   const long long Nc = 2LL * h->ws_nrhs, big = (long long)o * v * o * Nc;
   dev_free(h, h->XU, big); dev_free(h, h->Z, big); dev_free(h, h->V, big);
   dev_free(h, h->Y, (long long)h->Q * o * Nc);
@@ -208,7 +220,8 @@ static int ensure_workspace(gfcc_ctx* h, int nrhs, bool need_abi_vecs) {
   if (h->ws_nrhs != nrhs) {
     if (h->ws_nrhs) free_workspace(h);
     const long long Nc = 2LL * nrhs, big = (long long)o * v * o * Nc;
-    h->panel_ni = choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes);
+    h->panel_ni = h->opt_engine == 1 ? oz_choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes)
+                                     : choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes);
     h->ws_nrhs = nrhs;
     TRY(dev_alloc(h, &h->XU, big)); TRY(dev_alloc(h, &h->Z, big)); TRY(dev_alloc(h, &h->V, big));
     TRY(dev_alloc(h, &h->Y, (long long)Q * o * Nc));
@@ -240,7 +253,8 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   // Every GEMM CTA owns a whole SM, so running the chains on separate streams lets the block scheduler fill the
   // ragged last wave of one panel GEMM with CTAs of another chain.  With per-launch GEMM timing on (profile_gemm)
   // the chains are serialised on the handle's stream so that the event brackets do not overlap.
-  const bool par = h->opt_overlap != 0 && !h->prof && h->sB && h->sC && h->KP2;
+  const bool oz = h->opt_engine == 1;
+  const bool par = !oz && h->opt_overlap != 0 && !h->prof && h->sB && h->sC && h->KP2;
   cudaStream_t s0 = h->stream, sB = par ? h->sB : s0, sC = par ? h->sC : s0;
   double* KPb = par ? h->KP2 : h->KP;
   struct Restore { gfcc_ctx* h; ~Restore() { h->cur = h->stream; } } restore{h};
@@ -270,7 +284,8 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     d.C = h->Z; d.sCm0 = ld;
     TRY(gemm(h, d));
   }
-  for (int i0 = 0; i0 < o; i0 += h->panel_ni) {
+  if (oz) TRY(sigma_ring_ozaki(h, nrhs));
+  for (int i0 = 0; i0 < o && !oz; i0 += h->panel_ni) {
     const int ni = std::min(h->panel_ni, o - i0);
     // ---- chain A: S8+S9 (+S3,S4 folded): panel of K2'[(i,a)][(m,e)], Z -= K2' XU
     h->cur = s0;
@@ -369,7 +384,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     CUDA_TRY(h, cudaStreamWaitEvent(s0, h->evC, 0));
   }
   // S11: Z[i][a][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]   (T2 blocks through the pair table, sign per block)
-  {
+  if (!oz) {
     GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
     d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
     d.tabs_even = ((long long)v * v) % 2 == 0;
@@ -767,7 +782,14 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "panel_bytes" && val > 0) { h->opt_panel_bytes = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
   else if (k == "overlap" && (val == 0 || val == 1)) { h->opt_overlap = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
-  else if (k == "profile_gemm") { h->prof = (val != 0); h->ev_used = 0; h->ev_flops.clear(); }
+  else if (k == "engine" && (val == 0 || val == 1)) { h->opt_engine = (int)val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
+  else if (k == "ozaki_slices" && val >= 2 && val <= OZ_MAX_SLICES) {
+    cudaStreamSynchronize(h->stream);
+    if (h->ws_nrhs) free_workspace(h);
+    oz_release(h, h->ozLvv); oz_release(h, h->ozLooT); oz_release(h, h->ozLov); h->oz_const_ready = false;
+    h->opt_oz_slices = (int)val;
+  }
+  else if (k == "profile_gemm") { h->prof = (val != 0); h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); }
   else { h->err = "gfcc_set_option: unknown key or invalid value: " + k; return GFCC_EINVAL; }
   return GFCC_OK;
 }
@@ -786,7 +808,25 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
   else if (k == "gemm_launches") *val = h->st_gemm_launches;
   else if (k == "kernel_launches") *val = h->st_kernel_launches;
   else if (k == "panel_ni") *val = h->panel_ni;
+  else if (k == "oz_gemms") *val = h->st_oz_gemms;
+  else if (k == "oz_fail") {
+    int hf = 0;
+    if (h->oz_fail && (cudaStreamSynchronize(h->stream) != cudaSuccess ||
+                       cudaMemcpy(&hf, h->oz_fail, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)) { h->err = "sync failed"; return GFCC_ECUDA; }
+    *val = hf;
+  }
   else if (k == "gmres_m_used") *val = h->sw.m;
+  else if (k == "oz_time_ms" || k == "oz_ops_timed" || k == "oz_flops_timed" || k == "oz_launches_timed") {
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "sync failed"; return GFCC_ECUDA; }
+    double ms = 0, ops = 0, fl = 0, n = 0;
+    for (size_t q = 0; q < h->ev_flops.size(); ++q) {
+      float t = 0;
+      if (h->ev_ops8[q] > 0 && cudaEventElapsedTime(&t, h->ev_pool[2 * q], h->ev_pool[2 * q + 1]) == cudaSuccess) {
+        ms += t; ops += h->ev_ops8[q]; fl += h->ev_flops[q]; n += 1;
+      }
+    }
+    *val = (k == "oz_time_ms") ? ms : (k == "oz_ops_timed") ? ops : (k == "oz_flops_timed") ? fl : n;
+  }
   else if (k == "gemm_time_ms" || k == "gemm_flops_timed" || k == "gemm_launches_timed" || k == "gemm_time_max_ms") {
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "sync failed"; return GFCC_ECUDA; }
     double ms = 0, fl = 0, mx = 0;
@@ -796,7 +836,7 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
     }
     *val = (k == "gemm_time_ms") ? ms : (k == "gemm_flops_timed") ? fl : (k == "gemm_time_max_ms") ? mx : (double)h->ev_flops.size();
   }
-  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = 0; }
+  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = 0; }
   else { h->err = "gfcc_get_stat: unknown key " + k; return GFCC_EINVAL; }
   return GFCC_OK;
 }

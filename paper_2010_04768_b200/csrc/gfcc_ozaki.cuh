@@ -35,13 +35,16 @@ constexpr int OZ_MAX_UNITS = 40;
 constexpr int OZ_MAX_PAIRS = 8;
 constexpr long long OZ_MAX_TERMS = 500000;                   // terms of magnitude <= 64*64 per int32 accumulator (< 2^31 / 2^12)
 
-// operand view: element (r, k), k = k1*K0 + k0  ->  base[(tab ? tab[k1] : k1*sK1) + r*sR + k0*sK0] * (sgn ? sgn[k1] : 1)
+// operand view: element (r, k), k = k1*K0 + k0  ->  base[(tab ? tab[k1] : k1*sK1) + r*sR + k0*sK0] * (sgn ? sgn[k1] : 1).
+// With Rb > 0 the rows come in blocks of Rb that each have their own table row: rb = r / Rb, r' = r % Rb,
+// element = base[tab[rb*tabR + k1] + r'*sR + k0*sK0] * sgn[rb*tabR + k1]   (the signed pair-packed T2 blocks of S11).
 struct OzOperand {
   const double* base = nullptr;
   long long sR = 0, sK0 = 0, sK1 = 0;
   const long long* tab = nullptr;
   const double* sgn = nullptr;
   int R = 0, K0 = 0, K1 = 1;
+  int Rb = 0, tabR = 0;
 };
 
 // sliced operand: S int8 matrices [S][Rpad][Kpad] (K-major) + per-row scale 2^(e-6) (0 for an all-zero row)
@@ -61,9 +64,11 @@ constexpr int OZ_TR = 64, OZ_TK = 64;
 
 __device__ __forceinline__ double oz_load(const OzOperand& a, int r, int k) {
   const int k1 = k / a.K0, k0 = k - k1 * a.K0;
-  const long long off = (a.tab ? a.tab[k1] : (long long)k1 * a.sK1) + (long long)r * a.sR + (long long)k0 * a.sK0;
+  int t = k1;
+  if (a.Rb > 0) { const int rb = r / a.Rb; r -= rb * a.Rb; t += rb * a.tabR; }
+  const long long off = (a.tab ? a.tab[t] : (long long)k1 * a.sK1) + (long long)r * a.sR + (long long)k0 * a.sK0;
   const double x = a.base[off];
-  return a.sgn ? x * a.sgn[k1] : x;
+  return a.sgn ? x * a.sgn[t] : x;
 }
 
 // amax[r] = max_k |x[r][k]| (as the bit pattern of a non-negative double, which orders like the value)
