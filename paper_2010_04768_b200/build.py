@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgfcc_b200.so")
 SOURCES = ["gfcc_lib.cu"]
-DEPS = ["gfcc_lib.cu", "gfcc_gemm.cuh", "gfcc_gemm_ws.cuh", "gfcc_kernels.cuh", "gfcc_solve.cuh", "gfcc_probe.cuh", "gfcc_mor.cuh", "gfcc_mor_host.inl", os.path.join("..", "..", "include", "gfcc.h")]
+DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".inl", ".h"))) + [os.path.join("..", "..", "include", "gfcc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

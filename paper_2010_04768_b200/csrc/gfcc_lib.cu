@@ -971,9 +971,18 @@ extern "C" int gfcc_dgemm_ozaki(void* stream, int M, int N, int K, double alpha,
     if (oz_slice(a, sa, st) != cudaSuccess || oz_slice(b, sb, st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     cudaEventRecord(ev[1], st);
     OzCDesc c; c.C = C; c.sCm0 = sCm; c.sCn0 = sCn; c.alpha = alpha; c.beta = beta;
-    if (oz_igemm(sa, sb, c, fail, st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    long long* dbg = nullptr;
+    if (getenv("GFCC_OZ_DEBUG")) { cudaMalloc(&dbg, 128); cudaMemsetAsync(dbg, 0, 128, st); }
+    if (oz_igemm(sa, sb, c, fail, st, 148, dbg) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     cudaEventRecord(ev[2], st);
     if (cudaStreamSynchronize(st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    if (dbg) {
+      long long hd[16];
+      cudaMemcpy(hd, dbg, 128, cudaMemcpyDeviceToHost); cudaFree(dbg);
+      fprintf(stderr, "   epilogue parts: transpose (incl. wait for TMEM data) %lld, C loads %lld, compute+stores %lld\n", hd[7], hd[8], hd[9]);
+      fprintf(stderr, "oz dbg (CTA 0, cycles): producer wait empty %lld | mma wait tempty %lld, wait full %lld | epilogue wait tfull %lld, "
+              "tmem ld %lld, whole epilogue %lld over %lld units\n", hd[0], hd[1], hd[2], hd[3], hd[4], hd[5], hd[6]);
+    }
     int hfail = 0;
     cudaMemcpy(&hfail, fail, sizeof(int), cudaMemcpyDeviceToHost);
     if (hfail) { rc = GFCC_ECUDA; break; }

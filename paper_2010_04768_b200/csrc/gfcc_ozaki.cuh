@@ -24,6 +24,7 @@
 #include <cstdint>
 #include <vector>
 #include <algorithm>
+#include <cstdlib>
 
 namespace gfcc {
 
@@ -206,16 +207,29 @@ __device__ __forceinline__ void oz_tmem_ld32(unsigned taddr, int (&v)[32]) {
 // one flush unit: npairs slice pairs of equal order g = s + t over the k-blocks [kb0, kb1), accumulated in ONE int32 tile
 struct OzUnit { short g, np; unsigned char s[OZ_MAX_PAIRS], t[OZ_MAX_PAIRS]; int kb0, kb1; };
 struct OzGemmParams {
-  int M, N, tiles_m, tiles_n, nunits;
+  int M, N, tiles_m, tiles_n, nunits, group_m;
   double alpha, beta;
   const double* sa; const double* sb;
   double* C; long long sCm0, sCm1; int Md; long long sCn0, sCn1; int Nd;
   int* fail;
+  long long* dbg;          // optional [8] cycle counters of CTA 0 (profiling aid; null in production)
   OzUnit u[OZ_MAX_UNITS];
 };
 
+// tile rasterisation: groups of group_m M-tiles sweep N (M fastest inside a group) so that the ~148 tiles in flight share
+// operand blocks through L2: working set = group_m A-blocks + 148/group_m B-blocks
+__device__ __forceinline__ void oz_tile_coords(int tile, int tiles_m, int tiles_n, int group_m, int& tm, int& tn) {
+  const int per_group = group_m * tiles_n;
+  const int g = tile / per_group;
+  const int first = g * group_m;
+  const int gsz = min(group_m, tiles_m - first);
+  const int r = tile - g * per_group;
+  tm = first + r % gsz;
+  tn = r / gsz;
+}
+
 constexpr unsigned OZ_A_BYTES = OZ_BM * OZ_BK, OZ_B_BYTES = OZ_BN * OZ_BK, OZ_STAGE_BYTES = OZ_A_BYTES + OZ_B_BYTES;
-constexpr size_t OZ_SMEM_BYTES = (size_t)OZ_STAGES * OZ_STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr size_t OZ_SMEM_BYTES = (size_t)OZ_STAGES * OZ_STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 4 * 32 * 33 * 4 /*epilogue transposes*/;
 // instruction descriptor: D = S32 (2 << 4), A = B = signed int8 (1 << 7, 1 << 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
 constexpr unsigned OZ_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(OZ_BN >> 3) << 17) | ((unsigned)(OZ_BM >> 4) << 24);
 
@@ -260,12 +274,16 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
       int stage = 0; unsigned phase = 0;
       bool ok = true;
       for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
-        const int m0 = (tile % p.tiles_m) * OZ_BM, n0 = (tile / p.tiles_m) * OZ_BN;
+        int tm, tn;
+        oz_tile_coords(tile, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+        const int m0 = tm * OZ_BM, n0 = tn * OZ_BN;
         for (int u = 0; u < p.nunits && ok; ++u) {
           const OzUnit& un = p.u[u];
           for (int pr = 0; pr < un.np && ok; ++pr)
             for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              const long long t0 = clock64();
               if (!(ok = oz_mbar_wait(&empty[stage], phase ^ 1, p.fail))) break;
+              if (p.dbg && blockIdx.x == 0) p.dbg[0] += clock64() - t0;
               uint8_t* sa = smem + (size_t)stage * OZ_STAGE_BYTES;
               oz_mbar_expect_tx(&full[stage], OZ_STAGE_BYTES);
               oz_tma_load_3d(sa, &tmA, &full[stage], kb * OZ_BK, m0, un.s[pr]);
@@ -285,13 +303,17 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
         for (int u = 0; u < p.nunits && ok; ++u, ++cnt) {
           const OzUnit& un = p.u[u];
           const unsigned buf = cnt & 1, use = cnt >> 1;
+          const long long t0 = clock64();
           if (!(ok = oz_mbar_wait(&tempty[buf], (use & 1) ^ 1, p.fail))) break;
+          if (p.dbg && blockIdx.x == 0) p.dbg[1] += clock64() - t0;
           oz_tc_fence_after();
           const unsigned tmem_d = tmem_base + buf * OZ_BN;
           unsigned acc = 0;
           for (int pr = 0; pr < un.np && ok; ++pr)
             for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              const long long t1 = clock64();
               if (!(ok = oz_mbar_wait(&full[stage], phase, p.fail))) break;
+              if (p.dbg && blockIdx.x == 0) p.dbg[2] += clock64() - t1;
               oz_tc_fence_after();
               const unsigned a_addr = oz_smem(smem + (size_t)stage * OZ_STAGE_BYTES);
               const uint64_t da = oz_smem_desc(a_addr), db = oz_smem_desc(a_addr + OZ_A_BYTES);
@@ -309,44 +331,76 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
     }
   } else {
     // ============================== epilogue warps: TMEM -> FP64 read-modify-write of C ==============================
+    // tcgen05.ld hands every lane 32 consecutive columns of ITS row; a [32][33] shared-memory transpose per warp turns that
+    // into "32 lanes = 32 consecutive columns of one row", so every global access of the read-modify-write is coalesced.
     const int quad = warp & 3;                      // TMEM lane quadrant this warp may access
-    const int rl = quad * 32 + lane;
+    int* tr = reinterpret_cast<int*>(smem + (size_t)OZ_STAGES * OZ_STAGE_BYTES + 256) + (warp - 2) * (32 * 33);
     unsigned cnt = 0;
     bool ok = true;
     for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
-      const int m0 = (tile % p.tiles_m) * OZ_BM, n0 = (tile / p.tiles_m) * OZ_BN;
-      const int row = m0 + rl;
+      int tm, tn;
+      oz_tile_coords(tile, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+      const int m0 = tm * OZ_BM, n0 = tn * OZ_BN;
+      const int row = m0 + quad * 32 + lane;        // the row this lane owns in TMEM
       const bool rok = row < p.M;
       const double rs0 = rok ? p.alpha * p.sa[row] : 0.0;
-      double* crow = p.C + (rok ? (long long)(row % p.Md) * p.sCm0 + (long long)(row / p.Md) * p.sCm1 : 0);
+      const long long roff = rok ? (long long)(row % p.Md) * p.sCm0 + (long long)(row / p.Md) * p.sCm1 : -1;
+      const int nrows = min(32, p.M - (m0 + quad * 32));     // valid rows of this warp's quadrant (may be <= 0)
       for (int u = 0; u < p.nunits && ok; ++u, ++cnt) {
         const unsigned buf = cnt & 1, use = cnt >> 1;
+        const long long t0 = clock64();
         ok = oz_mbar_wait(&tfull[buf], use & 1, p.fail);
         ok = __all_sync(0xffffffffu, ok);
         if (!ok) break;
         oz_tc_fence_after();
+        const long long t1 = clock64();
+        long long t_ld = 0, t_sts = 0, t_lg = 0, t_sg = 0;
         const double rs = rs0 * exp2((double)(-7 * p.u[u].g));
-        const bool first = (u == 0);
+        const bool load_c = !(u == 0 && p.beta == 0.0);
+        const double cb = (u == 0) ? p.beta : 1.0;
 #pragma unroll 1
         for (int c = 0; c < OZ_BN / 32; ++c) {
           int v[32];
+          const long long t2 = clock64();
           oz_tmem_ld32(tmem_base + ((unsigned)(quad * 32) << 16) + buf * OZ_BN + c * 32, v);
-          const int col0 = n0 + c * 32;
-          if (rok && col0 < p.N) {
+          t_ld += clock64() - t2;
+          const int col = n0 + c * 32 + lane;       // the column this lane owns after the transpose
+          if (n0 + c * 32 >= p.N || nrows <= 0) continue;
+          const long long t3 = clock64();
+          __syncwarp();
 #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const int col = col0 + j;
-              if (col < p.N) {
-                double* cp = crow + (long long)(col % p.Nd) * p.sCn0 + (long long)(col / p.Nd) * p.sCn1;
-                const double val = rs * p.sb[col] * (double)v[j];
-                if (first) *cp = (p.beta == 0.0) ? val : p.beta * (*cp) + val;
-                else *cp += val;
-              }
+          for (int j = 0; j < 32; ++j) tr[lane * 33 + j] = v[j];
+          __syncwarp();
+          const long long t4 = clock64();
+          t_sts += t4 - t3;
+          const bool cok = col < p.N;
+          const long long coff = cok ? (long long)(col % p.Nd) * p.sCn0 + (long long)(col / p.Nd) * p.sCn1 : 0;
+          const double sbv = cok ? __ldg(p.sb + col) : 0.0;
+          // all 32 coalesced row loads of the read-modify-write are issued before the first store (one memory round trip per chunk)
+          double cv[32];
+          long long ro[32];
+#pragma unroll
+          for (int r = 0; r < 32; ++r) {
+            ro[r] = __shfl_sync(0xffffffffu, roff, r);
+            cv[r] = (load_c && r < nrows && cok) ? __ldcs(p.C + ro[r] + coff) : 0.0;
+          }
+          const long long t5 = clock64();
+          t_lg += t5 - t4;
+#pragma unroll
+          for (int r = 0; r < 32; ++r) {
+            const double rsr = __shfl_sync(0xffffffffu, rs, r);
+            if (r < nrows && cok) {
+              const double val = rsr * sbv * (double)tr[r * 33 + lane];
+              __stcs(p.C + ro[r] + coff, load_c ? fma(cb, cv[r], val) : val);
             }
           }
+          t_sg += clock64() - t5;
         }
         oz_tc_fence_before();
         __syncwarp();
+        if (p.dbg && blockIdx.x == 0 && warp == 2 && lane == 0) {
+          p.dbg[3] += t1 - t0; p.dbg[4] += t_ld; p.dbg[5] += clock64() - t1; p.dbg[6] += 1; p.dbg[7] += t_sts; p.dbg[8] += t_lg; p.dbg[9] += t_sg;
+        }
         if (lane == 0) oz_mbar_arrive(&tempty[buf]);
       }
     }
@@ -415,7 +469,8 @@ struct OzCDesc {
 
 // C (+)= alpha * A * B^T from the sliced operands (A: M rows, B: N rows, common K).  `fail` is a device int (zeroed by the
 // caller) that the kernel raises if a pipeline wait times out.
-inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc& c, int* fail, cudaStream_t st, int num_sms = 148) {
+inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc& c, int* fail, cudaStream_t st, int num_sms = 148,
+                            long long* dbg = nullptr) {
   if (A.K != B.K || A.S != B.S || A.S < 1 || A.S > OZ_MAX_SLICES) return cudaErrorInvalidValue;
   static bool attr = false;
   if (!attr) {
@@ -432,6 +487,7 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
   p.C = c.C; p.sCm0 = c.sCm0; p.sCm1 = c.sCm1; p.Md = c.Md > 0 ? c.Md : A.R;
   p.sCn0 = c.sCn0; p.sCn1 = c.sCn1; p.Nd = c.Nd > 0 ? c.Nd : B.R;
   p.fail = fail;
+  p.dbg = dbg;
   // flush units: order g = S-1 .. 0 (small contributions first), pairs of one order chunked so that pairs * k-range fits int32
   const int S = A.S;
   const long long kblocks = A.Kpad / OZ_BK;
@@ -453,6 +509,11 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     }
   }
   p.nunits = nu;
+  p.group_m = std::max(1, std::min(p.tiles_m, 17));       // sqrt(148 * BN / BM): minimal L2 working set of the tiles in flight
+  {
+    const char* e = getenv("GFCC_OZ_GROUP_M");
+    if (e && atoi(e) > 0) p.group_m = std::min(p.tiles_m, atoi(e));
+  }
   const int grid = std::min(p.tiles_m * p.tiles_n, num_sms);
   if (grid < 1) return cudaSuccess;
   oz_igemm_kernel<<<grid, OZ_THREADS, OZ_SMEM_BYTES, st>>>(tmA, tmB, p);
