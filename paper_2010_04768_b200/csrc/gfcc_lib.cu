@@ -979,9 +979,8 @@ extern "C" int gfcc_dgemm_ozaki(void* stream, int M, int N, int K, double alpha,
     if (dbg) {
       long long hd[16];
       cudaMemcpy(hd, dbg, 128, cudaMemcpyDeviceToHost); cudaFree(dbg);
-      fprintf(stderr, "   epilogue parts: transpose (incl. wait for TMEM data) %lld, C loads %lld, compute+stores %lld\n", hd[7], hd[8], hd[9]);
       fprintf(stderr, "oz dbg (CTA 0, cycles): producer wait empty %lld | mma wait tempty %lld, wait full %lld | epilogue wait tfull %lld, "
-              "tmem ld %lld, whole epilogue %lld over %lld units\n", hd[0], hd[1], hd[2], hd[3], hd[4], hd[5], hd[6]);
+              "whole epilogue %lld over %lld units\n", hd[0], hd[1], hd[2], hd[3], hd[5], hd[6]);
     }
     int hfail = 0;
     cudaMemcpy(&hfail, fail, sizeof(int), cudaMemcpyDeviceToHost);

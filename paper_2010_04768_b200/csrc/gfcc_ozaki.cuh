@@ -354,25 +354,19 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
         if (!ok) break;
         oz_tc_fence_after();
         const long long t1 = clock64();
-        long long t_ld = 0, t_sts = 0, t_lg = 0, t_sg = 0;
         const double rs = rs0 * exp2((double)(-7 * p.u[u].g));
         const bool load_c = !(u == 0 && p.beta == 0.0);
         const double cb = (u == 0) ? p.beta : 1.0;
 #pragma unroll 1
         for (int c = 0; c < OZ_BN / 32; ++c) {
           int v[32];
-          const long long t2 = clock64();
           oz_tmem_ld32(tmem_base + ((unsigned)(quad * 32) << 16) + buf * OZ_BN + c * 32, v);
-          t_ld += clock64() - t2;
           const int col = n0 + c * 32 + lane;       // the column this lane owns after the transpose
           if (n0 + c * 32 >= p.N || nrows <= 0) continue;
-          const long long t3 = clock64();
           __syncwarp();
 #pragma unroll
           for (int j = 0; j < 32; ++j) tr[lane * 33 + j] = v[j];
           __syncwarp();
-          const long long t4 = clock64();
-          t_sts += t4 - t3;
           const bool cok = col < p.N;
           const long long coff = cok ? (long long)(col % p.Nd) * p.sCn0 + (long long)(col / p.Nd) * p.sCn1 : 0;
           const double sbv = cok ? __ldg(p.sb + col) : 0.0;
@@ -384,8 +378,6 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
             ro[r] = __shfl_sync(0xffffffffu, roff, r);
             cv[r] = (load_c && r < nrows && cok) ? __ldcs(p.C + ro[r] + coff) : 0.0;
           }
-          const long long t5 = clock64();
-          t_lg += t5 - t4;
 #pragma unroll
           for (int r = 0; r < 32; ++r) {
             const double rsr = __shfl_sync(0xffffffffu, rs, r);
@@ -394,12 +386,11 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
               __stcs(p.C + ro[r] + coff, load_c ? fma(cb, cv[r], val) : val);
             }
           }
-          t_sg += clock64() - t5;
         }
         oz_tc_fence_before();
         __syncwarp();
         if (p.dbg && blockIdx.x == 0 && warp == 2 && lane == 0) {
-          p.dbg[3] += t1 - t0; p.dbg[4] += t_ld; p.dbg[5] += clock64() - t1; p.dbg[6] += 1; p.dbg[7] += t_sts; p.dbg[8] += t_lg; p.dbg[9] += t_sg;
+          p.dbg[3] += t1 - t0; p.dbg[5] += clock64() - t1; p.dbg[6] += 1;
         }
         if (lane == 0) oz_mbar_arrive(&tempty[buf]);
       }
@@ -409,6 +400,159 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
   __syncthreads();
   if (warp == 1) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "r"(512u) : "memory");
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// short-K variant: 128 x 128 tiles, 8 epilogue warps that keep the FP64 sums of ALL flush units of a tile in registers
+// (64 per thread) and write C once -- no read-modify-write of C between units.  Used when K is so short that the
+// per-unit read-modify-write of the 128 x 256 kernel would dominate (the (ov x ov) panel builds from the Cholesky vectors,
+// K = Q).  Same pipeline otherwise: 1 TMA warp, 1 MMA warp, two TMEM accumulators of 128 columns.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int OZR_BN = 128, OZR_STAGES = 6, OZR_THREADS = 320;
+constexpr unsigned OZR_B_BYTES = OZR_BN * OZ_BK, OZR_STAGE_BYTES = OZ_A_BYTES + OZR_B_BYTES;
+constexpr size_t OZR_SMEM_BYTES = (size_t)OZR_STAGES * OZR_STAGE_BYTES + 1024 + 256;
+constexpr unsigned OZR_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(OZR_BN >> 3) << 17) | ((unsigned)(OZ_BM >> 4) << 24);
+
+__global__ void __launch_bounds__(OZR_THREADS, 1) oz_igemm_regacc_kernel(const __grid_constant__ CUtensorMap tmA,
+                                                                         const __grid_constant__ CUtensorMap tmB,
+                                                                         const __grid_constant__ OzGemmParams p) {
+  extern __shared__ uint8_t oz_smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)oz_smem_raw + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)OZR_STAGES * OZR_STAGE_BYTES);
+  uint64_t* full = bars;
+  uint64_t* empty = bars + OZR_STAGES;
+  uint64_t* tfull = bars + 2 * OZR_STAGES;
+  uint64_t* tempty = tfull + 2;
+  unsigned* tmem_slot = reinterpret_cast<unsigned*>(tempty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < OZR_STAGES; ++s) { oz_mbar_init(&full[s], 1); oz_mbar_init(&empty[s], 1); }
+    oz_mbar_init(&tfull[0], 1); oz_mbar_init(&tfull[1], 1);
+    oz_mbar_init(&tempty[0], 8); oz_mbar_init(&tempty[1], 8);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(&tmA) : "memory");
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(&tmB) : "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(oz_smem(tmem_slot)), "r"(256u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+  }
+  oz_tc_fence_before();
+  __syncthreads();
+  oz_tc_fence_after();
+  const unsigned tmem_base = *tmem_slot;
+  const int ntiles = p.tiles_m * p.tiles_n;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      int stage = 0; unsigned phase = 0;
+      bool ok = true;
+      for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+        int tm, tn;
+        oz_tile_coords(tile, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+        const int m0 = tm * OZ_BM, n0 = tn * OZR_BN;
+        for (int u = 0; u < p.nunits && ok; ++u) {
+          const OzUnit& un = p.u[u];
+          for (int pr = 0; pr < un.np && ok; ++pr)
+            for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              if (!(ok = oz_mbar_wait(&empty[stage], phase ^ 1, p.fail))) break;
+              uint8_t* sa = smem + (size_t)stage * OZR_STAGE_BYTES;
+              oz_mbar_expect_tx(&full[stage], OZR_STAGE_BYTES);
+              oz_tma_load_3d(sa, &tmA, &full[stage], kb * OZ_BK, m0, un.s[pr]);
+              oz_tma_load_3d(sa + OZ_A_BYTES, &tmB, &full[stage], kb * OZ_BK, n0, un.t[pr]);
+              if (++stage == OZR_STAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      int stage = 0; unsigned phase = 0;
+      unsigned cnt = 0;
+      bool ok = true;
+      for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+        for (int u = 0; u < p.nunits && ok; ++u, ++cnt) {
+          const OzUnit& un = p.u[u];
+          const unsigned buf = cnt & 1, use = cnt >> 1;
+          if (!(ok = oz_mbar_wait(&tempty[buf], (use & 1) ^ 1, p.fail))) break;
+          oz_tc_fence_after();
+          const unsigned tmem_d = tmem_base + buf * OZR_BN;
+          unsigned acc = 0;
+          for (int pr = 0; pr < un.np && ok; ++pr)
+            for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              if (!(ok = oz_mbar_wait(&full[stage], phase, p.fail))) break;
+              oz_tc_fence_after();
+              const unsigned a_addr = oz_smem(smem + (size_t)stage * OZR_STAGE_BYTES);
+              const uint64_t da = oz_smem_desc(a_addr), db = oz_smem_desc(a_addr + OZ_A_BYTES);
+#pragma unroll
+              for (int k = 0; k < OZ_BK / 32; ++k) {
+                oz_mma_i8(tmem_d, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), OZR_IDESC, acc);
+                acc = 1;
+              }
+              oz_tc_commit(&empty[stage]);
+              if (++stage == OZR_STAGES) { stage = 0; phase ^= 1; }
+            }
+          if (ok) oz_tc_commit(&tfull[buf]);
+        }
+      }
+    }
+  } else {
+    // epilogue: warp (quad, half) owns TMEM lanes quad*32.. and columns half*64..; 64 FP64 sums per thread live across the units
+    const int quad = warp & 3, half = (warp - 2) >> 2;
+    unsigned cnt = 0;
+    bool ok = true;
+    for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+      int tm, tn;
+      oz_tile_coords(tile, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+      const int row = tm * OZ_BM + quad * 32 + lane, col0 = tn * OZR_BN + half * 64;
+      double acc[64];
+#pragma unroll
+      for (int j = 0; j < 64; ++j) acc[j] = 0.0;
+      for (int u = 0; u < p.nunits && ok; ++u, ++cnt) {
+        const unsigned buf = cnt & 1, use = cnt >> 1;
+        ok = oz_mbar_wait(&tfull[buf], use & 1, p.fail);
+        ok = __all_sync(0xffffffffu, ok);
+        if (!ok) break;
+        oz_tc_fence_after();
+        const double sg = exp2((double)(-7 * p.u[u].g));      // exact power of two
+        const unsigned taddr = tmem_base + ((unsigned)(quad * 32) << 16) + buf * OZR_BN + half * 64;
+        {
+          int v[32];
+          oz_tmem_ld32(taddr, v);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) acc[j] = fma(sg, (double)v[j], acc[j]);
+          oz_tmem_ld32(taddr + 32, v);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) acc[32 + j] = fma(sg, (double)v[j], acc[32 + j]);
+        }
+        oz_tc_fence_before();
+        __syncwarp();
+        if (lane == 0) oz_mbar_arrive(&tempty[buf]);
+      }
+      if (!ok) break;
+      if (row < p.M && col0 < p.N) {
+        const double rs = p.alpha * p.sa[row];
+        double* crow = p.C + (long long)(row % p.Md) * p.sCm0 + (long long)(row / p.Md) * p.sCm1;
+        int q = col0 / p.Nd, r = col0 - q * p.Nd;
+#pragma unroll
+        for (int j = 0; j < 64; ++j) {
+          if (col0 + j < p.N) {
+            double* cp = crow + (long long)r * p.sCn0 + (long long)q * p.sCn1;
+            const double val = rs * __ldg(p.sb + col0 + j) * acc[j];
+            __stcs(cp, p.beta == 0.0 ? val : fma(p.beta, __ldcs(cp), val));
+          }
+          if (++r == p.Nd) { r = 0; ++q; }
+        }
+      }
+    }
+  }
+  oz_tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "r"(256u) : "memory");
   }
 }
 
@@ -478,11 +622,24 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     if (e != cudaSuccess) return e;
     attr = true;
   }
+  // short K: the register-accumulating 128 x 128 kernel (C written once); long K: 128 x 256 tiles with per-unit read-modify-write
+  bool regacc = A.K <= 16384;
+  {
+    const char* e = getenv("GFCC_OZ_REGACC");
+    if (e) regacc = atoi(e) != 0;
+  }
+  const int bn = regacc ? OZR_BN : OZ_BN;
+  static bool attr2 = false;
+  if (regacc && !attr2) {
+    cudaError_t e = cudaFuncSetAttribute(oz_igemm_regacc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OZR_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr2 = true;
+  }
   CUtensorMap tmA, tmB;
-  if (!oz_make_map(&tmA, A, OZ_BM) || !oz_make_map(&tmB, B, OZ_BN)) return cudaErrorUnknown;
+  if (!oz_make_map(&tmA, A, OZ_BM) || !oz_make_map(&tmB, B, bn)) return cudaErrorUnknown;
   OzGemmParams p;
   p.M = A.R; p.N = B.R;
-  p.tiles_m = (A.R + OZ_BM - 1) / OZ_BM; p.tiles_n = (B.R + OZ_BN - 1) / OZ_BN;
+  p.tiles_m = (A.R + OZ_BM - 1) / OZ_BM; p.tiles_n = (B.R + bn - 1) / bn;
   p.alpha = c.alpha; p.beta = c.beta; p.sa = A.scale; p.sb = B.scale;
   p.C = c.C; p.sCm0 = c.sCm0; p.sCm1 = c.sCm1; p.Md = c.Md > 0 ? c.Md : A.R;
   p.sCn0 = c.sCn0; p.sCn1 = c.sCn1; p.Nd = c.Nd > 0 ? c.Nd : B.R;
@@ -509,14 +666,15 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     }
   }
   p.nunits = nu;
-  p.group_m = std::max(1, std::min(p.tiles_m, 17));       // sqrt(148 * BN / BM): minimal L2 working set of the tiles in flight
+  p.group_m = std::max(1, std::min(p.tiles_m, regacc ? 12 : 17));   // sqrt(148 * BN / BM): minimal L2 working set of the tiles in flight
   {
     const char* e = getenv("GFCC_OZ_GROUP_M");
     if (e && atoi(e) > 0) p.group_m = std::min(p.tiles_m, atoi(e));
   }
   const int grid = std::min(p.tiles_m * p.tiles_n, num_sms);
   if (grid < 1) return cudaSuccess;
-  oz_igemm_kernel<<<grid, OZ_THREADS, OZ_SMEM_BYTES, st>>>(tmA, tmB, p);
+  if (regacc) oz_igemm_regacc_kernel<<<grid, OZR_THREADS, OZR_SMEM_BYTES, st>>>(tmA, tmB, p);
+  else oz_igemm_kernel<<<grid, OZ_THREADS, OZ_SMEM_BYTES, st>>>(tmA, tmB, p);
   return cudaGetLastError();
 }
 
