@@ -1,7 +1,7 @@
 """Micro-benchmarks of the building blocks (B200): FP64 DMMA ceiling, the GEMM engine on square and on the sigma-shaped
 problems of a config, HBM copy.  Used for the roofline notes in DESIGN.md / profiles/ and as the short command ncu wraps.
 
-    python -m paper_2010_04768_b200.microbench [--probe] [--square N] [--sigma-shapes CFG] [--reps R]
+    python -m paper_2010_04768_b200.microbench [--probe] [--square N] [--sigma-shapes CFG] [--ozaki-shapes CFG] [--slices S] [--reps R]
 """
 import argparse
 import json
@@ -33,11 +33,28 @@ def time_gemm(M, N, K, ta=False, tb=False, reps=3):
     return {"M": M, "N": N, "K": K, "ta": ta, "tb": tb, "ms": best, "tflops": 2.0 * M * N * K / best / 1e9}
 
 
+def time_ozaki(M, N, K, ta=False, S=7, reps=2):
+    """gfcc_dgemm_ozaki (INT8 tensor-core engine): CUDA-event times of the slicing passes and of the tcgen05 kernel"""
+    A = torch.randn((K, M) if ta else (M, K), dtype=torch.float64, device="cuda")
+    B = torch.randn((K, N), dtype=torch.float64, device="cuda")
+    C = torch.zeros((M, N), dtype=torch.float64, device="cuda")
+    Av = A.t() if ta else A
+    best = (1e30, 1e30)
+    for _ in range(reps):
+        _, ms_s, ms_g = g.gfcc_dgemm_ozaki(Av, B, C, nslices=S, return_times=True)
+        best = min(best, (ms_g, ms_s))
+    ms_g, ms_s = best
+    return {"M": M, "N": N, "K": K, "ta": ta, "slices": S, "ms_gemm": ms_g, "ms_slice": ms_s,
+            "fp64_equiv_tflops": 2.0 * M * N * K / ms_g / 1e9, "int8_tops": 2.0 * M * N * K * (S * (S + 1) // 2) / ms_g / 1e9}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--probe", action="store_true")
     ap.add_argument("--square", type=int, default=0)
     ap.add_argument("--sigma-shapes", type=int, default=0)
+    ap.add_argument("--ozaki-shapes", type=int, default=0)
+    ap.add_argument("--slices", type=int, default=7)
     ap.add_argument("--reps", type=int, default=3)
     a = ap.parse_args()
     out = {}
@@ -69,6 +86,18 @@ def main():
             r = time_gemm(M, N, K, ta, tb, a.reps)
             r["name"] = name
             out["sigma_shapes"].append(r)
+    if a.ozaki_shapes:
+        o, v, Q, nrhs = SHAPES[a.ozaki_shapes]
+        ov, ld = o * v, o * 2 * nrhs
+        ni = max(1, min(o, int(4.2e9 // (ov * 8 * v))))
+        shapes = [("S8  K2 panel build (short K: register-accumulating kernel)", ni * o, v * v, Q, True),
+                  ("S10 K4 panel build (short K)", ov, ni * v, Q, True),
+                  ("S9  Z -= K2 XU (panel; long K: 128 x 256 kernel)", ni * v, ld, ov, False)]
+        out["ozaki_shapes"] = []
+        for name, M, N, K, ta in shapes:
+            r = time_ozaki(M, N, K, ta, a.slices, max(1, min(a.reps, 2)))
+            r["name"] = name
+            out["ozaki_shapes"].append(r)
     print(json.dumps(out))
 
 

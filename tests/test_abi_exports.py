@@ -34,6 +34,9 @@ def test_sass_is_sm100a_dmma():
     assert "sm_100a" in out
     assert "DMMA.8x8x4" in out            # FP64 tensor-core MMA
     assert "LDGSTS" in out                # cp.async shared-memory staging
+    assert "UTCIMMA" in out               # tcgen05.mma kind::i8 (INT8 engine)
+    assert "UTMALDG" in out               # TMA loads
+    assert "LDTM" in out                  # tcgen05.ld (TMEM -> registers)
 
 
 def test_no_cpu_fallback():

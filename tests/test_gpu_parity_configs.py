@@ -48,9 +48,12 @@ def _triples(o, v, n, seed):
     return np.array(out[:n], dtype=np.int32)
 
 
-def _sampled_sigma_check(cfg, nrhs, rsel, ntrip, s1rows):
+def _sampled_sigma_check(cfg, nrhs, rsel, ntrip, s1rows, engine=0):
     g, c, s, h, orc = _setup(cfg)
     o, v = c["o"], c["v"]
+    if engine:                                   # INT8 tensor-core engine instead of the graded FP64 DMMA engine
+        g.gfcc_set_option(h, "engine", 1)
+        g.gfcc_set_option(h, "panel_bytes", 4.2e9)
     X1, X2 = gi.trial_vectors(o, v, nrhs, gi.seed_of(cfg), "cuda")
     w = np.resize(np.linspace(c["wlo"], c["whi"], c["nw"]), nrhs)
     S1, S2 = g.gfcc_sigma_ip(h, w, c["eta"], X1, X2)
@@ -70,6 +73,8 @@ def _sampled_sigma_check(cfg, nrhs, rsel, ntrip, s1rows):
     G2t = np.stack([S2h[:, j, i, a] for (i, j, a) in trip], axis=0)
     assert np.array_equal(G2t, -G2)
     assert float(S2[:, torch.arange(o), torch.arange(o), :].abs().max().item()) == 0.0
+    if engine:
+        assert g.gfcc_get_stat(h, "oz_gemms") > 0 and g.gfcc_get_stat(h, "oz_fail") == 0
     g.gfcc_destroy(h)
     assert e1 < TOL_SIGMA and e2 < TOL_SIGMA, (e1, e2)
     return e1, e2
@@ -131,3 +136,12 @@ def test_config1_solve_residual_rows_and_G():
 def test_large_config_sigma_sampled_rows(cfg, ntrip):
     c = gi.CONFIGS[cfg]
     _sampled_sigma_check(cfg, c["np"] * c["nw"], [c["np"] * c["nw"] - 1], ntrip, [c["o"] - 1])
+
+
+@pytest.mark.skipif(os.environ.get("GFCC_TEST_LARGE", "0") != "1", reason="set GFCC_TEST_LARGE=1 (needs >100 GB host memory, ~15 min)")
+@pytest.mark.parametrize("cfg,nrhs,ntrip", [(3, 32, 3), (4, 8, 2)])
+def test_large_config_sigma_sampled_rows_engine_ozaki(cfg, nrhs, ntrip):
+    """the INT8 tensor-core engine at full size (config 4 with an 8-RHS batch: its extra 20 GB of digit slices beside the 16-RHS
+    batch, the borrowed T2/Lambda2 and this test's own X and sigma copies would not fit 180 GB)"""
+    c = gi.CONFIGS[cfg]
+    _sampled_sigma_check(cfg, nrhs, [nrhs - 1], ntrip, [c["o"] - 1], engine=1)
