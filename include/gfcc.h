@@ -136,6 +136,22 @@ int gfcc_mor_extend(gfcc_handle h, int nx, const void* X1, const void* X2, doubl
 int gfcc_mor_solve(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, void* G, double* A);
 long long gfcc_mor_get(gfcc_handle h, const char* name, double* out);
 
+/* ---- Level loop of the retarded GFCCSD workflow (Alg. 1, Eq. 12-13) ----
+ * Fine grid w_k = wmin + k*dw, k = 0..n_fine-1 with n_fine = round((wmax-wmin)/dw)+1 (the caller passes it; checked).
+ * Level 1 solves Eq. 5 at 3 grid points (both ends and the middle, Eq. 12) for every target p [host][np] with the batched
+ * GMRES of gfcc_solve_ip (stop test tol), orthogonalises the solutions into the MOR subspace (droptol), projects, and
+ * evaluates G^ and A on the whole fine grid (gfcc_mor_*).  Level L > 1 adds the middle grid points of at most 2^(L-1)
+ * intervals between sampled points (Eq. 12): all of them at level 2, afterwards those on which A moved by more than
+ * spec_tol * max|A| between the two latest models, largest change first (readings 26-27; the paper cites Ref. 100
+ * for the strategy and prints only the counts).  Stops when no interval qualifies, after L_max = floor(log2((wmax-wmin)/dw))
+ * levels (Eq. 13) or after max_levels (> 0) levels.  The handle's MOR subspace is reset and left holding the final model.
+ * Outputs (host): A [n_fine] spectral function, G [n_fine][np][np] complex (nullable; host or device), level_of [n_fine]
+ * (level at which the grid point was sampled, 0 = never), *levels_out, *m_out (nullable).  Synchronous.
+ * Returns GFCC_ENOCONV if some GMRES solve stopped at its iteration limit (results are still written).                   */
+int gfcc_spectral_adaptive(gfcc_handle h, int np, const int* p, double wmin, double wmax, double dw, double eta,
+                           double tol, double spec_tol, int max_levels, double droptol, int n_fine, double* A,
+                           void* G, int* level_of, int* levels_out, int* m_out);
+
 const char* gfcc_last_error(gfcc_handle h);
 int gfcc_destroy(gfcc_handle h);
 

@@ -24,7 +24,7 @@ GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_intermediate", "gfcc_last_error",
            "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
-           "gfcc_mor_get"]
+           "gfcc_mor_get", "gfcc_spectral_adaptive"]
 
 
 class GfccError(RuntimeError):
@@ -69,6 +69,7 @@ def lib():
     L.gfcc_mor_solve.argtypes = [vp, ci, ip, ci, dp, cd, vp, dp]
     L.gfcc_mor_get.argtypes = [vp, ctypes.c_char_p, vp]
     L.gfcc_mor_get.restype = cll
+    L.gfcc_spectral_adaptive.argtypes = [vp, ci, ip, cd, cd, cd, cd, cd, cd, ci, cd, ci, dp, vp, ip, ip, ip]
     for name in EXPORTS:
         if name not in ("gfcc_get_intermediate", "gfcc_last_error", "gfcc_mor_get"):
             getattr(L, name).restype = ci
@@ -224,6 +225,23 @@ def gfcc_solve_ip(h, p, omega, eta, tol, return_x=False, allow_noconv=False):
                              G.ctypes.data)
     _check(h, rc, allow)
     return G
+
+
+def gfcc_spectral_adaptive(h, p, wmin, wmax, dw, eta, tol, spec_tol=1e-3, max_levels=0, droptol=1e-8, allow_noconv=False):
+    """Alg. 1 level loop with adaptive midpoint refinement (include/gfcc.h).  Returns dict(w, A, G, level_of, levels, m)."""
+    _torch()
+    pa = np.ascontiguousarray(p, dtype=np.int32)
+    n = int(round((wmax - wmin) / dw)) + 1
+    A = np.zeros(n, dtype=np.float64)
+    G = np.zeros((n, len(pa), len(pa)), dtype=np.complex128)
+    lev = np.zeros(n, dtype=np.int32)
+    levels, m = ctypes.c_int(), ctypes.c_int()
+    rc = lib().gfcc_spectral_adaptive(h.ptr, len(pa), pa.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), float(wmin), float(wmax),
+                                      float(dw), float(eta), float(tol), float(spec_tol), int(max_levels), float(droptol), n,
+                                      A.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), G.ctypes.data,
+                                      lev.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), ctypes.byref(levels), ctypes.byref(m))
+    _check(h, rc, (GFCC_ENOCONV,) if allow_noconv else ())
+    return {"w": wmin + dw * np.arange(n), "A": A, "G": G, "level_of": lev, "levels": levels.value, "m": m.value}
 
 
 def gfcc_dgemm(A, B, C=None, alpha=1.0, beta=0.0, stream=0):

@@ -1088,3 +1088,4 @@ extern "C" int gfcc_solve_ip(gfcc_handle h, int np, const int* p, int nw, const 
 }
 
 #include "gfcc_mor_host.inl"
+#include "gfcc_workflow_host.inl"
