@@ -231,7 +231,8 @@ def gfcc_spectral_adaptive(h, p, wmin, wmax, dw, eta, tol, spec_tol=1e-3, max_le
     """Alg. 1 level loop with adaptive midpoint refinement (include/gfcc.h).  Returns dict(w, A, G, level_of, levels, m)."""
     _torch()
     pa = np.ascontiguousarray(p, dtype=np.int32)
-    n = int(round((wmax - wmin) / dw)) + 1
+    n = int(round((wmax - wmin) / dw)) + 1 if dw > 0 else 0
+    n = max(n, 1)                                  # the library rejects an empty window or a grid of fewer than 3 points
     A = np.zeros(n, dtype=np.float64)
     G = np.zeros((n, len(pa), len(pa)), dtype=np.complex128)
     lev = np.zeros(n, dtype=np.int32)

@@ -64,6 +64,7 @@ struct OzSliced {
 constexpr int OZ_TR = 64, OZ_TK = 64;
 
 __device__ __forceinline__ double oz_load(const OzOperand& a, int r, int k) {
+  if (a.K1 == 1 && a.Rb == 0 && !a.tab && !a.sgn) return a.base[(long long)r * a.sR + (long long)k * a.sK0];     // plain strided operand
   const int k1 = k / a.K0, k0 = k - k1 * a.K0;
   int t = k1;
   if (a.Rb > 0) { const int rb = r / a.Rb; r -= rb * a.Rb; t += rb * a.tabR; }
@@ -72,20 +73,36 @@ __device__ __forceinline__ double oz_load(const OzOperand& a, int r, int k) {
   return a.sgn ? x * a.sgn[t] : x;
 }
 
-// amax[r] = max_k |x[r][k]| (as the bit pattern of a non-negative double, which orders like the value)
+// amax[r] = max_k |x[r][k]| (as the bit pattern of a non-negative double, which orders like the value).
+// Each thread keeps a running maximum for the row(s) it owns: in the row-fast case a thread always sees the same row of the
+// 64 x 64 tile, in the k-fast case a warp covers 32 consecutive k of one row and reduces by shuffles.
 __global__ void __launch_bounds__(256) k_oz_absmax(OzOperand a, unsigned long long* __restrict__ amax) {
   __shared__ unsigned long long smax[OZ_TR];
   const int r0 = blockIdx.y * OZ_TR, k0 = blockIdx.x * OZ_TK, K = a.K0 * a.K1;
   if (threadIdx.x < OZ_TR) smax[threadIdx.x] = 0ull;
   __syncthreads();
   const bool kfast = (a.sK0 == 1);
-  for (int idx = threadIdx.x; idx < OZ_TR * OZ_TK; idx += 256) {
-    const int rl = kfast ? idx / OZ_TK : idx % OZ_TR, kl = kfast ? idx % OZ_TK : idx / OZ_TR;
-    const int r = r0 + rl, k = k0 + kl;
-    if (r < a.R && k < K) {
-      const unsigned long long b = (unsigned long long)__double_as_longlong(fabs(oz_load(a, r, k)));
-      if (b > smax[rl]) atomicMax(&smax[rl], b);
+  if (kfast) {
+    const int kl = threadIdx.x & 63, k = k0 + kl;
+#pragma unroll 4
+    for (int i = 0; i < OZ_TR / 4; ++i) {
+      const int rl = (threadIdx.x >> 6) + 4 * i, r = r0 + rl;
+      double m = (r < a.R && k < K) ? fabs(oz_load(a, r, k)) : 0.0;
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, off));
+      if ((threadIdx.x & 31) == 0 && m > 0.0) atomicMax(&smax[rl], (unsigned long long)__double_as_longlong(m));
     }
+  } else {
+    const int rl = threadIdx.x & 63, r = r0 + rl;
+    double m = 0.0;
+    if (r < a.R) {
+#pragma unroll 4
+      for (int i = 0; i < OZ_TK / 4; ++i) {
+        const int k = k0 + (threadIdx.x >> 6) + 4 * i;
+        if (k < K) m = fmax(m, fabs(oz_load(a, r, k)));
+      }
+    }
+    if (m > 0.0) atomicMax(&smax[rl], (unsigned long long)__double_as_longlong(m));
   }
   __syncthreads();
   if (threadIdx.x < OZ_TR && r0 + threadIdx.x < a.R && smax[threadIdx.x] != 0ull) atomicMax(&amax[r0 + threadIdx.x], smax[threadIdx.x]);

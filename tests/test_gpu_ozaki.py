@@ -125,8 +125,10 @@ def test_solve_small_engine_ozaki():
     g.gfcc_destroy(h)
 
 
-def test_config1_sigma_sampled_rows_engine_ozaki():
-    """config 1 at full size (o=40, v=160, Q=600, 64-RHS batch) on the INT8 engine against the row-sampled oracle"""
+@pytest.mark.parametrize("slices", [7, 6])
+def test_config1_sigma_sampled_rows_engine_ozaki(slices):
+    """config 1 at full size (o=40, v=160, Q=600, 64-RHS batch) on the INT8 engine against the row-sampled oracle; 7 digit
+    slices is the default, 6 (21 instead of 28 digit products, ~1e-11 per GEMM) still meets the 1e-10 bar"""
     import paper_2010_04768_b200 as g
     cfg, nrhs, rsel = 1, 64, [0, 17, 63]
     c = gi.CONFIGS[cfg]
@@ -134,6 +136,7 @@ def test_config1_sigma_sampled_rows_engine_ozaki():
     s = gi.make_config(cfg, "cuda")
     host = {k: s[k].cpu().numpy() for k in ("fock", "T1", "T2p", "L1", "L2p", "Lchol")}
     h = g.gfcc_create(o, v, c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+    g.gfcc_set_option(h, "ozaki_slices", slices)
     g.gfcc_set_option(h, "engine", 1)
     orc = oracle.Oracle(o, v, c["Q"], host["fock"], host["T1"], host["T2p"], host["L1"], host["L2p"], host["Lchol"], oracle.MODE_ROWS)
     X1, X2 = gi.trial_vectors(o, v, nrhs, gi.seed_of(cfg), "cuda")

@@ -32,6 +32,7 @@ def _setup(cfg):
     host = {k: s[k].cpu().numpy() for k in ("fock", "T1", "T2p", "L1", "L2p", "Lchol")}
     h = g.gfcc_create(c["o"], c["v"], c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
     del s["Lchol"]
+    torch.cuda.empty_cache()                     # hand the 14 GB of Lchol (config 4) back to the driver, not to torch's cache
     orc = oracle.Oracle(c["o"], c["v"], c["Q"], host["fock"], host["T1"], host["T2p"], host["L1"], host["L2p"], host["Lchol"],
                         oracle.MODE_ROWS)
     return g, c, s, h, orc
