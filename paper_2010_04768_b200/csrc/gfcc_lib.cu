@@ -963,17 +963,17 @@ extern "C" int gfcc_dgemm_ozaki(void* stream, int M, int N, int K, double alpha,
     if (cudaMalloc(&sa.q, sa.bytes()) != cudaSuccess || cudaMalloc(&sb.q, sb.bytes()) != cudaSuccess ||
         cudaMalloc(&sa.scale, (size_t)M * 8) != cudaSuccess || cudaMalloc(&sb.scale, (size_t)N * 8) != cudaSuccess ||
         cudaMalloc(&sa.amax, (size_t)M * 8) != cudaSuccess || cudaMalloc(&sb.amax, (size_t)N * 8) != cudaSuccess ||
-        cudaMalloc(&fail, sizeof(int)) != cudaSuccess) { rc = GFCC_ENOMEM; break; }
+        cudaMalloc(&fail, 2 * sizeof(int)) != cudaSuccess) { rc = GFCC_ENOMEM; break; }
     for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     if (rc) break;
-    cudaMemsetAsync(fail, 0, sizeof(int), st);
+    cudaMemsetAsync(fail, 0, 2 * sizeof(int), st);
     cudaEventRecord(ev[0], st);
     if (oz_slice(a, sa, st) != cudaSuccess || oz_slice(b, sb, st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     cudaEventRecord(ev[1], st);
     OzCDesc c; c.C = C; c.sCm0 = sCm; c.sCn0 = sCn; c.alpha = alpha; c.beta = beta;
     long long* dbg = nullptr;
     if (getenv("GFCC_OZ_DEBUG")) { cudaMalloc(&dbg, 128); cudaMemsetAsync(dbg, 0, 128, st); }
-    if (oz_igemm(sa, sb, c, fail, st, 148, dbg) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    if (oz_igemm(sa, sb, c, fail, st, 148, dbg, reinterpret_cast<unsigned*>(fail) + 1) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     cudaEventRecord(ev[2], st);
     if (cudaStreamSynchronize(st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     if (dbg) {

@@ -230,6 +230,7 @@ struct OzGemmParams {
   double* C; long long sCm0, sCm1; int Md; long long sCn0, sCn1; int Nd;
   int* fail;
   long long* dbg;          // optional [8] cycle counters of CTA 0 (profiling aid; null in production)
+  unsigned* sync; int sync_every, steps_per_tile;   // optional producer rendezvous every sync_every k-blocks (L2 co-scheduling)
   OzUnit u[OZ_MAX_UNITS];
 };
 
@@ -290,6 +291,12 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
     if (lane == 0) {
       int stage = 0; unsigned phase = 0;
       bool ok = true;
+      // rendezvous of the producers: the tiles in flight share operand blocks only through L2, which the operand stream turns
+      // over every ~10 us; CTAs that drift apart by more than that re-fetch from DRAM.  Every sync_every k-blocks each producer
+      // waits until all CTAs that still have work have issued the same k-block count (all CTAs are co-resident: 1 per SM).
+      long long gstep = 0, next_sync = p.sync_every;
+      unsigned expected = 0;
+      const long long q_steps = (long long)(ntiles / (int)gridDim.x) * p.steps_per_tile, rem = ntiles % (int)gridDim.x;
       for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
         int tm, tn;
         oz_tile_coords(tile, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
@@ -298,6 +305,15 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
           const OzUnit& un = p.u[u];
           for (int pr = 0; pr < un.np && ok; ++pr)
             for (int kb = un.kb0; kb < un.kb1; ++kb) {
+              if (p.sync_every > 0 && gstep == next_sync) {
+                expected += (unsigned)((gstep < q_steps) ? (long long)gridDim.x : rem);     // CTAs that reach this point
+                atomicAdd(p.sync, 1u);
+                for (long long spin = 0; *(volatile unsigned*)p.sync < expected; ++spin)
+                  if (spin > (1ll << 24)) { atomicExch(p.fail, 2); ok = false; break; }
+                if (!ok) break;
+                next_sync += p.sync_every;
+              }
+              ++gstep;
               const long long t0 = clock64();
               if (!(ok = oz_mbar_wait(&empty[stage], phase ^ 1, p.fail))) break;
               if (p.dbg && blockIdx.x == 0) p.dbg[0] += clock64() - t0;
@@ -631,7 +647,7 @@ struct OzCDesc {
 // C (+)= alpha * A * B^T from the sliced operands (A: M rows, B: N rows, common K).  `fail` is a device int (zeroed by the
 // caller) that the kernel raises if a pipeline wait times out.
 inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc& c, int* fail, cudaStream_t st, int num_sms = 148,
-                            long long* dbg = nullptr) {
+                            long long* dbg = nullptr, unsigned* sync_buf = nullptr) {
   if (A.K != B.K || A.S != B.S || A.S < 1 || A.S > OZ_MAX_SLICES) return cudaErrorInvalidValue;
   static bool attr = false;
   if (!attr) {
@@ -662,6 +678,7 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
   p.sCn0 = c.sCn0; p.sCn1 = c.sCn1; p.Nd = c.Nd > 0 ? c.Nd : B.R;
   p.fail = fail;
   p.dbg = dbg;
+  p.sync = nullptr; p.sync_every = 0; p.steps_per_tile = 0;
   // flush units: order g = S-1 .. 0 (small contributions first), pairs of one order chunked so that pairs * k-range fits int32
   const int S = A.S;
   const long long kblocks = A.Kpad / OZ_BK;
@@ -690,6 +707,18 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
   }
   const int grid = std::min(p.tiles_m * p.tiles_n, num_sms);
   if (grid < 1) return cudaSuccess;
+  {
+    long long spt = 0;
+    for (int u = 0; u < p.nunits; ++u) spt += (long long)p.u[u].np * (p.u[u].kb1 - p.u[u].kb0);
+    p.steps_per_tile = (int)spt;
+    static int sync_every = -1;
+    if (sync_every < 0) { const char* e = getenv("GFCC_OZ_SYNC"); sync_every = e ? atoi(e) : 0; }
+    if (!regacc && sync_every > 0 && sync_buf) {
+      cudaError_t e = cudaMemsetAsync(sync_buf, 0, sizeof(unsigned), st);
+      if (e != cudaSuccess) return e;
+      p.sync = sync_buf; p.sync_every = sync_every;
+    }
+  }
   if (regacc) oz_igemm_regacc_kernel<<<grid, OZR_THREADS, OZR_SMEM_BYTES, st>>>(tmA, tmB, p);
   else oz_igemm_kernel<<<grid, OZ_THREADS, OZ_SMEM_BYTES, st>>>(tmA, tmB, p);
   return cudaGetLastError();

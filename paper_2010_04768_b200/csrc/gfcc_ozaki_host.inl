@@ -46,7 +46,7 @@ static int oz_gemm(gfcc_ctx* h, const OzSliced& A, const OzSliced& B, const OzCD
     while (h->ev_pool.size() < h->ev_used + 2) { cudaEvent_t e; CUDA_TRY(h, cudaEventCreate(&e)); h->ev_pool.push_back(e); }
     CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used], h->cur));
   }
-  CUDA_TRY(h, oz_igemm(A, B, c, h->oz_fail, h->cur));
+  CUDA_TRY(h, oz_igemm(A, B, c, h->oz_fail, h->cur, 148, nullptr, reinterpret_cast<unsigned*>(h->oz_fail) + 1));
   if (timed) {
     CUDA_TRY(h, cudaEventRecord(h->ev_pool[h->ev_used + 1], h->cur));
     h->ev_used += 2;
