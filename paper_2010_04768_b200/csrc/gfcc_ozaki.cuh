@@ -712,7 +712,7 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     for (int u = 0; u < p.nunits; ++u) spt += (long long)p.u[u].np * (p.u[u].kb1 - p.u[u].kb0);
     p.steps_per_tile = (int)spt;
     static int sync_every = -1;
-    if (sync_every < 0) { const char* e = getenv("GFCC_OZ_SYNC"); sync_every = e ? atoi(e) : 0; }
+    if (sync_every < 0) { const char* e = getenv("GFCC_OZ_SYNC"); sync_every = e ? atoi(e) : 256; }   // 0 switches it off
     if (!regacc && sync_every > 0 && sync_buf) {
       cudaError_t e = cudaMemsetAsync(sync_buf, 0, sizeof(unsigned), st);
       if (e != cudaSuccess) return e;
