@@ -79,6 +79,24 @@ def test_ozaki_gemm_slices_and_zero_rows():
         g.gfcc_dgemm_ozaki(dev(A), dev(B), nslices=9)
 
 
+@pytest.mark.parametrize("M,N,K", [(300, 520, 20000), (2560, 2560, 17000), (1000, 700, 140000)])
+def test_ozaki_gemm_long_k_kernel(M, N, K):
+    """K > 16384 selects the 128 x 256 read-modify-write kernel with the producer rendezvous (more tiles than SMs with a ragged
+    last round, K long enough that one flush unit holds fewer pairs, ragged M/N/K); reference: torch FP64 matmul on the device"""
+    import paper_2010_04768_b200 as g
+    gen = torch.Generator(device="cuda").manual_seed(M + N + K)
+    A = torch.randn((M, K), dtype=torch.float64, device="cuda", generator=gen)
+    B = torch.randn((K, N), dtype=torch.float64, device="cuda", generator=gen)
+    C0 = torch.randn((M, N), dtype=torch.float64, device="cuda", generator=gen)
+    C = C0.clone()
+    g.gfcc_dgemm_ozaki(A, B, C, alpha=-1.0, beta=1.0, nslices=7)
+    ref = C0 - A @ B
+    assert float((C - ref).abs().max() / ref.abs().max()) < 1e-12
+    C = g.gfcc_dgemm_ozaki(A, B, nslices=7)
+    ref = A @ B
+    assert float((C - ref).abs().max() / ref.abs().max()) < 1e-12
+
+
 def _make_pair(s):
     import paper_2010_04768_b200 as g
     orc = oracle.Oracle(s["o"], s["v"], s["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"], oracle.MODE_DEF)
