@@ -222,7 +222,9 @@ __device__ __forceinline__ void oz_tmem_ld32(unsigned taddr, int (&v)[32]) {
 }
 
 // one flush unit: npairs slice pairs of equal order g = s + t over the k-blocks [kb0, kb1), accumulated in ONE int32 tile
-struct OzUnit { short g, np; unsigned char s[OZ_MAX_PAIRS], t[OZ_MAX_PAIRS]; int kb0, kb1; };
+// (short-K kernel: np ENTRIES, each one A slice s[e] against up to two B slices: low nibble of t[e] = t0 + 1 -> accumulator of
+//  order g, high nibble = t1 + 1 -> accumulator of order g + 1, 0 = absent; ng = number of accumulators of the unit)
+struct OzUnit { short g, np, ng, pad_; unsigned char s[OZ_MAX_PAIRS], t[OZ_MAX_PAIRS]; int kb0, kb1; };
 struct OzGemmParams {
   int M, N, tiles_m, tiles_n, nunits, group_m;
   double alpha, beta;
@@ -440,10 +442,14 @@ __global__ void __launch_bounds__(OZ_THREADS, 1) oz_igemm_kernel(const __grid_co
 // short-K variant: 128 x 128 tiles, 8 epilogue warps that keep the FP64 sums of ALL flush units of a tile in registers
 // (64 per thread) and write C once -- no read-modify-write of C between units.  Used when K is so short that the
 // per-unit read-modify-write of the 128 x 256 kernel would dominate (the (ov x ov) panel builds from the Cholesky vectors,
-// K = Q).  Same pipeline otherwise: 1 TMA warp, 1 MMA warp, two TMEM accumulators of 128 columns.
+// K = Q).  Same pipeline otherwise: 1 TMA warp, 1 MMA warp, TMEM double-buffered.
+// A 128 x 128 tile needs 32 KB of operands per k-block and digit pair, which at the full INT8 rate is the whole L2 -> SM port; so
+// a flush unit covers TWO neighbouring orders (g, g+1) and every A_s block that lands in shared memory is multiplied with both
+// B_(g-s) and B_(g+1-s), into two TMEM accumulators: 3 operand blocks per 2 digit products instead of 4 (44 instead of 56 loads
+// per k-block for 7 slices).
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int OZR_BN = 128, OZR_STAGES = 6, OZR_THREADS = 320;
-constexpr unsigned OZR_B_BYTES = OZR_BN * OZ_BK, OZR_STAGE_BYTES = OZ_A_BYTES + OZR_B_BYTES;
+constexpr int OZR_BN = 128, OZR_STAGES = 4, OZR_THREADS = 320;
+constexpr unsigned OZR_B_BYTES = OZR_BN * OZ_BK, OZR_STAGE_BYTES = OZ_A_BYTES + 2 * OZR_B_BYTES;
 constexpr size_t OZR_SMEM_BYTES = (size_t)OZR_STAGES * OZR_STAGE_BYTES + 1024 + 256;
 constexpr unsigned OZR_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(OZR_BN >> 3) << 17) | ((unsigned)(OZ_BM >> 4) << 24);
 
@@ -470,7 +476,7 @@ __global__ void __launch_bounds__(OZR_THREADS, 1) oz_igemm_regacc_kernel(const _
     asm volatile("prefetch.tensormap [%0];\n" ::"l"(&tmB) : "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(oz_smem(tmem_slot)), "r"(256u) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(oz_smem(tmem_slot)), "r"(512u) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
   }
   oz_tc_fence_before();
@@ -493,9 +499,11 @@ __global__ void __launch_bounds__(OZR_THREADS, 1) oz_igemm_regacc_kernel(const _
             for (int kb = un.kb0; kb < un.kb1; ++kb) {
               if (!(ok = oz_mbar_wait(&empty[stage], phase ^ 1, p.fail))) break;
               uint8_t* sa = smem + (size_t)stage * OZR_STAGE_BYTES;
-              oz_mbar_expect_tx(&full[stage], OZR_STAGE_BYTES);
+              const int t0 = (un.t[pr] & 15) - 1, t1 = (un.t[pr] >> 4) - 1;
+              oz_mbar_expect_tx(&full[stage], OZ_A_BYTES + ((t0 >= 0) + (t1 >= 0)) * OZR_B_BYTES);
               oz_tma_load_3d(sa, &tmA, &full[stage], kb * OZ_BK, m0, un.s[pr]);
-              oz_tma_load_3d(sa + OZ_A_BYTES, &tmB, &full[stage], kb * OZ_BK, n0, un.t[pr]);
+              if (t0 >= 0) oz_tma_load_3d(sa + OZ_A_BYTES, &tmB, &full[stage], kb * OZ_BK, n0, t0);
+              if (t1 >= 0) oz_tma_load_3d(sa + OZ_A_BYTES + OZR_B_BYTES, &tmB, &full[stage], kb * OZ_BK, n0, t1);
               if (++stage == OZR_STAGES) { stage = 0; phase ^= 1; }
             }
         }
@@ -512,22 +520,27 @@ __global__ void __launch_bounds__(OZR_THREADS, 1) oz_igemm_regacc_kernel(const _
           const unsigned buf = cnt & 1, use = cnt >> 1;
           if (!(ok = oz_mbar_wait(&tempty[buf], (use & 1) ^ 1, p.fail))) break;
           oz_tc_fence_after();
-          const unsigned tmem_d = tmem_base + buf * OZR_BN;
-          unsigned acc = 0;
-          for (int pr = 0; pr < un.np && ok; ++pr)
+          const unsigned tmem_d0 = tmem_base + buf * (2 * OZR_BN), tmem_d1 = tmem_d0 + OZR_BN;
+          unsigned acc0 = 0, acc1 = 0;
+          for (int pr = 0; pr < un.np && ok; ++pr) {
+            const bool has0 = (un.t[pr] & 15) != 0, has1 = (un.t[pr] >> 4) != 0;
             for (int kb = un.kb0; kb < un.kb1; ++kb) {
               if (!(ok = oz_mbar_wait(&full[stage], phase, p.fail))) break;
               oz_tc_fence_after();
               const unsigned a_addr = oz_smem(smem + (size_t)stage * OZR_STAGE_BYTES);
-              const uint64_t da = oz_smem_desc(a_addr), db = oz_smem_desc(a_addr + OZ_A_BYTES);
+              const uint64_t da = oz_smem_desc(a_addr), db0 = oz_smem_desc(a_addr + OZ_A_BYTES),
+                             db1 = oz_smem_desc(a_addr + OZ_A_BYTES + OZR_B_BYTES);
 #pragma unroll
               for (int k = 0; k < OZ_BK / 32; ++k) {
-                oz_mma_i8(tmem_d, da + (uint64_t)(2 * k), db + (uint64_t)(2 * k), OZR_IDESC, acc);
-                acc = 1;
+                if (has0) oz_mma_i8(tmem_d0, da + (uint64_t)(2 * k), db0 + (uint64_t)(2 * k), OZR_IDESC, acc0 | (unsigned)(k > 0));
+                if (has1) oz_mma_i8(tmem_d1, da + (uint64_t)(2 * k), db1 + (uint64_t)(2 * k), OZR_IDESC, acc1 | (unsigned)(k > 0));
               }
+              if (has0) acc0 = 1;
+              if (has1) acc1 = 1;
               oz_tc_commit(&empty[stage]);
               if (++stage == OZR_STAGES) { stage = 0; phase ^= 1; }
             }
+          }
           if (ok) oz_tc_commit(&tfull[buf]);
         }
       }
@@ -550,9 +563,9 @@ __global__ void __launch_bounds__(OZR_THREADS, 1) oz_igemm_regacc_kernel(const _
         ok = __all_sync(0xffffffffu, ok);
         if (!ok) break;
         oz_tc_fence_after();
-        const double sg = exp2((double)(-7 * p.u[u].g));      // exact power of two
-        const unsigned taddr = tmem_base + ((unsigned)(quad * 32) << 16) + buf * OZR_BN + half * 64;
-        {
+        double sg = exp2((double)(-7 * p.u[u].g));            // exact power of two
+        unsigned taddr = tmem_base + ((unsigned)(quad * 32) << 16) + buf * (2 * OZR_BN) + half * 64;
+        for (int a = 0; a < p.u[u].ng; ++a, taddr += OZR_BN, sg *= 0.0078125) {
           int v[32];
           oz_tmem_ld32(taddr, v);
 #pragma unroll
@@ -585,7 +598,7 @@ __global__ void __launch_bounds__(OZR_THREADS, 1) oz_igemm_regacc_kernel(const _
   oz_tc_fence_before();
   __syncthreads();
   if (warp == 1) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "r"(256u) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "r"(512u) : "memory");
   }
 }
 
@@ -656,10 +669,10 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     attr = true;
   }
   // short K: the register-accumulating 128 x 128 kernel (C written once); long K: 128 x 256 tiles with per-unit read-modify-write
-  bool regacc = A.K <= 16384;
+  bool regacc = A.K <= 16384;     // (<= 8 entries per accumulator x K x 64^2 stays far below 2^31)
   {
     const char* e = getenv("GFCC_OZ_REGACC");
-    if (e) regacc = atoi(e) != 0;
+    if (e) regacc = atoi(e) != 0 && A.Kpad <= 65536;
   }
   const int bn = regacc ? OZR_BN : OZ_BN;
   static bool attr2 = false;
@@ -696,6 +709,23 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
         OzUnit& un = p.u[nu++];
         un.g = (short)g; un.np = 0; un.kb0 = (int)kb0; un.kb1 = (int)std::min(kblocks, kb0 + kb_chunk);
         while (s <= g && un.np < pairs_per_unit) { un.s[un.np] = (unsigned char)s; un.t[un.np] = (unsigned char)(g - s); ++un.np; ++s; }
+      }
+    }
+  }
+  if (regacc) {
+    // short-K kernel: one unit per pair of neighbouring orders (g, g+1) -- (0), (1,2), (3,4), ... for odd S, (0,1), (2,3), ... for
+    // even S -- smallest contributions first; entry s multiplies A_s with B_(g-s) and B_(g+1-s)
+    nu = 0;
+    for (int g1 = S - 1; g1 >= 0; g1 -= 2) {
+      const int g0 = (g1 >= 1) ? g1 - 1 : 0, ng = (g1 >= 1) ? 2 : 1;
+      OzUnit& un = p.u[nu++];
+      un.g = (short)g0; un.ng = (short)ng; un.np = 0; un.pad_ = 0; un.kb0 = 0; un.kb1 = (int)kblocks;
+      const int top = (ng == 2) ? g1 : g0;
+      for (int sA = 0; sA <= top; ++sA) {
+        const int t0 = g0 - sA, t1 = (ng == 2) ? g1 - sA : -1;
+        un.s[un.np] = (unsigned char)sA;
+        un.t[un.np] = (unsigned char)(((t0 >= 0) ? t0 + 1 : 0) | (((t1 >= 0) ? t1 + 1 : 0) << 4));
+        ++un.np;
       }
     }
   }
