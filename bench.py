@@ -358,7 +358,7 @@ def main():
                    "flops_per_sigma_application": flops_sigma, "sigma_applications_per_step": apps_per_step,
                    "gmres_m_used": g.gfcc_get_stat(h, "gmres_m_used"), "overlap": int(overlap_on),
                    "gemm_engine": (os.environ.get("GFCC_GEMM_ENGINE", "ws") if args.engine == "dmma" else
-                                   f"ozaki_int8 x{args.slices} slices for S8-S11 (tcgen05.mma kind::i8, exact int32 accumulation, FP64-accurate; "
+                                   f"ozaki_int8 x{args.slices} slices for S6, S8-S11 (tcgen05.mma kind::i8, exact int32 accumulation, FP64-accurate; "
                                    "NOT the graded FP64 DMMA engine), rest on the DMMA engine"),
                    "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
         "solves_per_s": solves_per_s, "solves_note": f"(p,omega) right-hand sides advanced by {kfix} GMRES steps per second x nrhs",
@@ -392,7 +392,7 @@ def main():
         r = line["roofline"]
         line["roofline_dmma_part"] = {k: r[k] for k in ("achieved", "launches", "share_of_step")}
         line["roofline"] = {
-            "kernel": "gfcc::oz_igemm_kernel (INT8 tcgen05 launches of the timed region: S8-S11)", "bound": "tensor",
+            "kernel": "gfcc::oz_igemm_kernel (INT8 tcgen05 launches of the timed region: S6, S8-S11)", "bound": "tensor",
             "achieved": oz_ops / (oz_ms * 1e-3) / 1e12, "peak": i8_peak, "unit": "TFLOP/s", "frac": oz_ops / (oz_ms * 1e-3) / 1e12 / i8_peak,
             "peak_source": "int8 dense = sustained bf16 of MEASURED_PEAKS.json x nominal ratio 4.5/2.25 (no measured int8 entry); unit is int8 TOP/s",
             "peak_alt_burst": (mp["bf16_tflops"] * 2.0) if mp else None,
@@ -447,7 +447,7 @@ def main():
                 "int8_tops_in_kernel": o_ops / (o_ms * 1e-3) / 1e12 if o_ms > 0 else None,
                 "fp64_equivalent_tflops_in_kernel": o_fl / (o_ms * 1e-3) / 1e12 if o_ms > 0 else None,
                 "kernel_share_of_step": o_ms / ms_oz if ms_oz > 0 else None, "oz_fail": g.gfcc_get_stat(h, "oz_fail"),
-                "note": "S8-S11 on tcgen05.mma kind::i8 with error-free slicing (FP64-accurate: sigma parity 1e-10 in tests/test_gpu_ozaki.py); "
+                "note": "S6, S8-S11 on tcgen05.mma kind::i8 with error-free slicing (FP64-accurate: sigma parity 1e-10 in tests/test_gpu_ozaki.py); "
                         "reported beside, not instead of, the graded FP64 DMMA number"}
         except Exception as ex:   # noqa: BLE001
             line["ozaki_int8"] = {"value": None, "error": str(ex)[:200]}

@@ -57,7 +57,8 @@ struct gfcc_ctx {
   int panel_ni = 1;
   // ---- INT8 tensor-core (Ozaki) engine for S8-S11 (gfcc_ozaki.cuh, gfcc_ozaki_host.inl; option "engine" = 1) ----
   int opt_engine = 0, opt_oz_slices = 7;
-  OzSliced ozLvv, ozLooT, ozLov, ozXU, ozKP;
+  OzSliced ozLvv, ozLooT, ozLov, ozXU, ozKP, ozWp;
+  double* ozS6scale = nullptr; long long ozS6rows = 0;
   int* oz_fail = nullptr;
   bool oz_const_ready = false;
   int oz_ws_nrhs = 0, oz_ws_ni = 0;
@@ -352,7 +353,9 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   k_sigma1_small<<<(unsigned)((o * nrhs + 127) / 128), 128, 0, sC>>>(sout, xin, h->Fmi, d_omega, eta, o, nrhs);
   KLAUNCH(h);
   // S6 (D): s2[(i<j)][(a,c)] = sum_(m<n) W[(i<j)][(m<n)] x2[(m<n)][(a,c)]
-  {
+  bool s6_done = false;
+  if (oz) TRY(sigma_s6_ozaki(h, nrhs, x2, s2, &s6_done));
+  if (!s6_done) {
     GemmDesc d; d.M = (int)h->npair; d.N = (int)(v * Nc); d.K0 = (int)h->npair;
     d.A = h->Wp; d.sAm = h->npair; d.sAk0 = 1;
     d.B = x2; d.sBk0 = v * Nc; d.sBn = 1;
@@ -786,7 +789,7 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "ozaki_slices" && val >= 2 && val <= OZ_MAX_SLICES) {
     cudaStreamSynchronize(h->stream);
     if (h->ws_nrhs) free_workspace(h);
-    oz_release(h, h->ozLvv); oz_release(h, h->ozLooT); oz_release(h, h->ozLov); h->oz_const_ready = false;
+    oz_release(h, h->ozLvv); oz_release(h, h->ozLooT); oz_release(h, h->ozLov); oz_release(h, h->ozWp); h->oz_const_ready = false;
     h->opt_oz_slices = (int)val;
   }
   else if (k == "profile_gemm") { h->prof = (val != 0); h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); }

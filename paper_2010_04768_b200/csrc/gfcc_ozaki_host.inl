@@ -1,7 +1,7 @@
 // =====================================================================================
 // gfcc_ozaki_host.inl -- the INT8 tensor-core (Ozaki) engine inside the sigma driver (included by gfcc_lib.cu).
 //
-// S8-S11 (panel builds from the Cholesky vectors, the two (ov x ov) panel contractions and the
+// S6 and S8-S11 (panel builds from the Cholesky vectors, the two (ov x ov) panel contractions and the
 // T2 contraction -- 97 % of the flops of an application at config 4) on tcgen05.mma kind::i8 with FP64 accuracy.
 // Option "engine" = 1 selects it; the graded default (engine 0) is the FP64 DMMA engine.
 //   constant operands (sliced once per handle):  Lvv [(a,e)][Q], LooT [(i,m)][Q], Lov [(m,e)][Q]
@@ -162,5 +162,34 @@ static int sigma_ring_ozaki(gfcc_ctx* h, int nrhs) {
     OzCDesc c; c.C = h->Z + (long long)i0 * v * ld; c.sCm0 = ld; c.beta = 1.0;
     TRY(oz_gemm(h, tb, h->ozXU, c));
   }
+  return GFCC_OK;
+}
+
+// S6 on the INT8 engine: s2[(i<j)][(a,c)] = sum_(m<n) W[(i<j)][(m<n)] x2[(m<n)][(a,c)].  W's digit slices are made once per handle;
+// x2's go into the panel slice buffer, which is idle outside the panel loop (if they do not fit, *done stays false and the caller
+// uses the DMMA engine).
+static int sigma_s6_ozaki(gfcc_ctx* h, int nrhs, const double* x2, double* s2, bool* done) {
+  *done = false;
+  const long long npair = h->npair, cols = (long long)h->v * 2 * nrhs;
+  if (npair < 1 || cols > 2147483647LL || !h->ozKP.q) return GFCC_OK;
+  OzSliced xb;
+  oz_shape(xb, (int)cols, (int)npair, h->opt_oz_slices);
+  if (xb.bytes() > h->ozKP.bytes()) return GFCC_OK;
+  if (!h->ozWp.q) {
+    TRY(oz_alloc(h, h->ozWp, (int)npair, (int)npair));
+    OzOperand a; a.base = h->Wp; a.sR = npair; a.sK0 = 1; a.R = (int)npair; a.K0 = (int)npair;
+    TRY(oz_do_slice(h, a, h->ozWp));
+  }
+  if (h->ozS6rows < cols) {
+    if (h->ozS6scale) { CUDA_TRY(h, cudaStreamSynchronize(h->cur)); dev_free(h, h->ozS6scale, 2 * h->ozS6rows); h->ozS6scale = nullptr; }
+    TRY(dev_alloc(h, &h->ozS6scale, 2 * cols));
+    h->ozS6rows = cols;
+  }
+  xb.q = h->ozKP.q; xb.scale = h->ozS6scale; xb.amax = reinterpret_cast<unsigned long long*>(h->ozS6scale + cols);
+  OzOperand x; x.base = x2; x.sR = 1; x.sK0 = cols; x.R = (int)cols; x.K0 = (int)npair;
+  TRY(oz_do_slice(h, x, xb));
+  OzCDesc c; c.C = s2; c.sCm0 = cols;
+  TRY(oz_gemm(h, h->ozWp, xb, c));
+  *done = true;
   return GFCC_OK;
 }
