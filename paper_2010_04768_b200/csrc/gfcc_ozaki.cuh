@@ -87,22 +87,22 @@ __global__ void __launch_bounds__(256) k_oz_absmax(OzOperand a, unsigned long lo
 #pragma unroll 4
     for (int i = 0; i < OZ_TR / 4; ++i) {
       const int rl = (threadIdx.x >> 6) + 4 * i, r = r0 + rl;
-      double m = (r < a.R && k < K) ? fabs(oz_load(a, r, k)) : 0.0;
+      unsigned long long m = (r < a.R && k < K) ? ((unsigned long long)__double_as_longlong(oz_load(a, r, k)) & 0x7fffffffffffffffull) : 0ull;
 #pragma unroll
-      for (int off = 16; off > 0; off >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, off));
-      if ((threadIdx.x & 31) == 0 && m > 0.0) atomicMax(&smax[rl], (unsigned long long)__double_as_longlong(m));
+      for (int off = 16; off > 0; off >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, off));
+      if ((threadIdx.x & 31) == 0 && m != 0ull) atomicMax(&smax[rl], m);
     }
   } else {
     const int rl = threadIdx.x & 63, r = r0 + rl;
-    double m = 0.0;
+    unsigned long long m = 0ull;
     if (r < a.R) {
 #pragma unroll 4
       for (int i = 0; i < OZ_TK / 4; ++i) {
         const int k = k0 + (threadIdx.x >> 6) + 4 * i;
-        if (k < K) m = fmax(m, fabs(oz_load(a, r, k)));
+        if (k < K) m = max(m, (unsigned long long)__double_as_longlong(oz_load(a, r, k)) & 0x7fffffffffffffffull);
       }
     }
-    if (m > 0.0) atomicMax(&smax[rl], (unsigned long long)__double_as_longlong(m));
+    if (m != 0ull) atomicMax(&smax[rl], m);
   }
   __syncthreads();
   if (threadIdx.x < OZ_TR && r0 + threadIdx.x < a.R && smax[threadIdx.x] != 0ull) atomicMax(&amax[r0 + threadIdx.x], smax[threadIdx.x]);
