@@ -201,7 +201,7 @@ extern "C" int gfcc_mor_solve(gfcc_handle h, int np, const int* p, int nw, const
     for (int c0 = 0; c0 < m; c0 += Ncc) {
       const int cnt = std::min(Ncc, m - c0);
       k_mor_copy_cols<<<nblk(n * Ncc), 256, 0, st>>>(vec, Ncc, Ncc, h->mor_S + c0, cap, n, cnt); KLAUNCH(h);
-      dim3 grid(g_blocks, (Ncc + LG_CC - 1) / LG_CC);
+      dim3 grid((Ncc + LG_CC - 1) / LG_CC, g_blocks);
       k_lambda2_g<<<grid, 32 * LG_WARPS, smem, st>>>(gpart, h->L2p, vec, o, v, Ncc, h->npair); KLAUNCH(h);
       const long long ng = (long long)v * Ncc;
       k_g_reduce<<<(unsigned)((ng + 127) / 128), 128, 0, st>>>(gvec, gpart, g_blocks, ng); KLAUNCH(h);

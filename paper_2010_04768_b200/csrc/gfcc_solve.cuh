@@ -180,83 +180,89 @@ __global__ void k_backsolve(int m, int nrhs, const double2* __restrict__ R, cons
 }
 
 // ---- g[b][c] = sum_(i,j,a) lambda[i,j,b,a] x2[i,j,a][c] = 2 sum_(i<j) sum_a l_p[b,a] x_p[a][c]  (Lambda2 packed [pair][a<b]) ----
-// grid (pair blocks, column chunks of LG_CC real columns); gpart[blk][v][Nc].
-// Every element U[a][b] (a<b) of a pair's packed triangle is read ONCE, coalesced (a row of the triangle is contiguous in b),
-// as part of a 32 x 32 tile that a warp parks in shared memory; the tile then serves both roles of the antisymmetric block:
-//   g[b] -= sum_a U[a][b] x[a]   (lane = b, walks the tile's column)      g[a] += sum_b U[a][b] x[b]   (lane = a, walks its row)
-// with LG_CC register accumulators per lane, folded into the block's g accumulator by shared-memory atomics.
+// grid (column chunks of LG_CC real columns, pair blocks); gpart[blk][v][Nc].
+// The chunks of one pair stream are neighbours in launch order, run at the same time and share every Lambda2 block through L2 (one
+// DRAM read of Lambda2 per batch).  Inside a block every warp OWNS 32-row blocks R of the output (R = warp, warp + 8, ...), so the
+// sums live in registers across all pairs and nothing is accumulated with atomics:
+//   g[b in R] -= sum_(a < b) U[a][b] x[a]   lane = b, walks DOWN column b of the packed triangle: every load is coalesced across b
+//   g[a in R] += sum_(b > a) U[a][b] x[b]   lane = a, needs row a: 32 x 32 tiles are read coalesced (along b) into shared memory
+//                                           and walked transposed
 constexpr int LG_CC = 8;
 constexpr int LG_WARPS = 8;
-constexpr int LG_TS = 33;                 // padded tile stride: row and column walks are both bank-conflict free
+constexpr int LG_NQ = 4;                  // output row blocks per warp and pass (one pass covers v <= 32 * 8 * 4 = 1024)
+constexpr int LG_TS = 33;                 // padded tile stride: the transposed walk is bank-conflict free
 inline int lg_vpad(int v) { return (v + 31) / 32 * 32; }
 inline size_t lambda2_g_smem_bytes(int v) {
-  return ((size_t)lg_vpad(v) * LG_CC + (size_t)v * LG_CC + (size_t)LG_WARPS * 32 * LG_TS) * sizeof(double);
+  return ((size_t)lg_vpad(v) * LG_CC + (size_t)LG_WARPS * 32 * LG_TS) * sizeof(double);
 }
 __global__ void __launch_bounds__(32 * LG_WARPS) k_lambda2_g(double* __restrict__ gpart, const double* __restrict__ L2p,
                                                               const double* __restrict__ vec, int o, int v, int Nc, long long npair) {
   extern __shared__ double sm[];
   const int vpad = (v + 31) / 32 * 32, nt = vpad / 32;
   double* xs = sm;                                   // [vpad][LG_CC], rows >= v are zero
-  double* ga = xs + (size_t)vpad * LG_CC;            // [v][LG_CC]
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  double* Ts = ga + (size_t)v * LG_CC + (size_t)warp * 32 * LG_TS;   // this warp's [32][LG_TS] tile
-  const int c0 = blockIdx.y * LG_CC;
+  double* Ts = xs + (size_t)vpad * LG_CC + (size_t)warp * 32 * LG_TS;   // this warp's [32][LG_TS] tile
+  const int c0 = blockIdx.x * LG_CC;
   const long long ntri = (long long)v * (v - 1) / 2;
-  for (int t = threadIdx.x; t < v * LG_CC; t += blockDim.x) ga[t] = 0.0;
   const double* x2 = vec + (long long)o * Nc;
-  for (long long pr = blockIdx.x; pr < npair; pr += gridDim.x) {
-    __syncthreads();
-    for (int t = threadIdx.x; t < vpad * LG_CC; t += blockDim.x) {
-      const int a = t / LG_CC, c = t % LG_CC;
-      xs[t] = (a < v && c0 + c < Nc) ? x2[(pr * v + a) * Nc + c0 + c] : 0.0;
-    }
-    __syncthreads();
-    const double* lp = L2p + pr * ntri;
-    int cnt = 0;
-    for (int ta = 0; ta < nt; ++ta)
-      for (int tb = ta; tb < nt; ++tb, ++cnt) {
-        if (cnt % LG_WARPS != warp) continue;
-        const int a0 = ta * 32, b0 = tb * 32, b = b0 + lane;
-        __syncwarp();
+  for (int rbase = 0; rbase < nt; rbase += LG_WARPS * LG_NQ) {
+    double acc[LG_NQ][LG_CC];
+#pragma unroll
+    for (int q = 0; q < LG_NQ; ++q)
+#pragma unroll
+      for (int c = 0; c < LG_CC; ++c) acc[q][c] = 0.0;
+    for (long long pr = blockIdx.y; pr < npair; pr += gridDim.y) {
+      __syncthreads();
+      for (int t = threadIdx.x; t < vpad * LG_CC; t += blockDim.x) {
+        const int a = t / LG_CC, c = t % LG_CC;
+        xs[t] = (a < v && c0 + c < Nc) ? x2[(pr * v + a) * Nc + c0 + c] : 0.0;
+      }
+      __syncthreads();
+      const double* lp = L2p + pr * ntri;
+#pragma unroll
+      for (int q = 0; q < LG_NQ; ++q) {
+        const int R = rbase + warp + LG_WARPS * q;
+        if (R >= nt) continue;                       // warp-uniform
+        const int me = R * 32 + lane;                // the output row this lane owns
+        // lambda[b, a] = -U[a][b] for a < b: column walk, coalesced across the lanes (b)
+        if (me < v) {
 #pragma unroll 8
-        for (int r = 0; r < 32; ++r) {
-          const int a = a0 + r;
-          Ts[r * LG_TS + lane] = (a < b && b < v) ? lp[tri_index(a, b, v)] : 0.0;
-        }
-        __syncwarp();
-        double acc[LG_CC];
+          for (int a = 0; a < me; ++a) {
+            const double u = lp[tri_index(a, me, v)];
+            const double* xr = xs + (size_t)a * LG_CC;
 #pragma unroll
-        for (int c = 0; c < LG_CC; ++c) acc[c] = 0.0;
+            for (int c = 0; c < LG_CC; ++c) acc[q][c] -= u * xr[c];
+          }
+        }
+        // lambda[a, b] = U[a][b] for b > a: row walk through transposed tiles
+        for (int tb = R; tb < nt; ++tb) {
+          const int b = tb * 32 + lane;
+          __syncwarp();
+#pragma unroll 8
+          for (int r = 0; r < 32; ++r) {
+            const int a = R * 32 + r;
+            Ts[r * LG_TS + lane] = (a < b && b < v) ? lp[tri_index(a, b, v)] : 0.0;
+          }
+          __syncwarp();
 #pragma unroll 4
-        for (int r = 0; r < 32; ++r) {               // lane = b: column walk
-          const double u = Ts[r * LG_TS + lane];
-          const double* xr = xs + (size_t)(a0 + r) * LG_CC;
+          for (int k = 0; k < 32; ++k) {
+            const double u = Ts[lane * LG_TS + k];
+            const double* xr = xs + (size_t)(tb * 32 + k) * LG_CC;
 #pragma unroll
-          for (int c = 0; c < LG_CC; ++c) acc[c] += u * xr[c];
-        }
-        if (b < v) {
-#pragma unroll
-          for (int c = 0; c < LG_CC; ++c) atomicAdd(&ga[b * LG_CC + c], -acc[c]);
-        }
-#pragma unroll
-        for (int c = 0; c < LG_CC; ++c) acc[c] = 0.0;
-#pragma unroll 4
-        for (int k = 0; k < 32; ++k) {               // lane = a: row walk
-          const double u = Ts[lane * LG_TS + k];
-          const double* xr = xs + (size_t)(b0 + k) * LG_CC;
-#pragma unroll
-          for (int c = 0; c < LG_CC; ++c) acc[c] += u * xr[c];
-        }
-        if (a0 + lane < v) {
-#pragma unroll
-          for (int c = 0; c < LG_CC; ++c) atomicAdd(&ga[(a0 + lane) * LG_CC + c], acc[c]);
+            for (int c = 0; c < LG_CC; ++c) acc[q][c] += u * xr[c];
+          }
         }
       }
-  }
-  __syncthreads();
-  for (int t = threadIdx.x; t < v * LG_CC; t += blockDim.x) {
-    const int b = t / LG_CC, c = t % LG_CC;
-    if (c0 + c < Nc) gpart[((long long)blockIdx.x * v + b) * Nc + c0 + c] = ga[t];
+    }
+#pragma unroll
+    for (int q = 0; q < LG_NQ; ++q) {
+      const int row = (rbase + warp + LG_WARPS * q) * 32 + lane;
+      if (row < v) {
+#pragma unroll
+        for (int c = 0; c < LG_CC; ++c)
+          if (c0 + c < Nc) gpart[((long long)blockIdx.y * v + row) * Nc + c0 + c] = acc[q][c];
+      }
+    }
   }
 }
 __global__ void k_g_reduce(double* __restrict__ gvec, const double* __restrict__ gpart, int nblk, long long n) {
@@ -477,7 +483,7 @@ inline int solve_run(SolveWs& s, const SolveCfg& c, const int* p_of_rhs, const d
   // ---- G assembly ----
   {
     const int Nc = 2 * nr;
-    dim3 grid(s.g_blocks, (Nc + LG_CC - 1) / LG_CC);
+    dim3 grid((Nc + LG_CC - 1) / LG_CC, s.g_blocks);
     const size_t smem = lambda2_g_smem_bytes(c.v);
     static bool attr_set = false;
     if (!attr_set) { cudaFuncSetAttribute(k_lambda2_g, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_set = true; }
