@@ -54,6 +54,7 @@ def parse():
                          "(SURVEY.md 8f row 2, reported separately)")
     ap.add_argument("--slices", type=int, default=7, help="digit slices of the ozaki engine (7: ~1e-13, 6: ~1e-11 per GEMM)")
     ap.add_argument("--no-ozaki-extra", action="store_true", help="skip the extra INT8-engine measurement appended to a dmma run")
+    ap.add_argument("--panel-bytes", type=float, default=0.0, help="byte budget of one (ov x ov) integral panel (default: library default)")
     ap.add_argument("--overlap", type=int, default=-1, help="1: run independent sigma panel chains on side streams (default: library default)")
     return ap.parse_args()
 
@@ -289,6 +290,8 @@ def main():
     g.gfcc_set_option(h, "max_batch", nrhs)
     if args.overlap >= 0:
         g.gfcc_set_option(h, "overlap", args.overlap)
+    if args.panel_bytes > 0:
+        g.gfcc_set_option(h, "panel_bytes", args.panel_bytes)
     if args.engine == "ozaki":
         g.gfcc_set_option(h, "ozaki_slices", args.slices)
         g.gfcc_set_option(h, "engine", 1)

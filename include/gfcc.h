@@ -90,7 +90,7 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *   "gmres_maxit"  maximum number of sigma applications per solve (default 1000)
  *   "gmres_fixed"  if > 0: run exactly this many Arnoldi steps in ONE cycle, no stop test (timing mode)
  *   "x0"           0: zero initial guess, 1: zeroth-order guess b/(omega - i eta + d) (default 1)
- *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3e9)
+ *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3.2e9: 5 occupied indices per panel at config 4)
  *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256)
  *   "overlap"      1: the K2 chain, the K4 chain and the small sigma terms run on three streams so that
  *                  CTAs of one chain fill the ragged last wave of another; 0 (default): everything on the handle's stream

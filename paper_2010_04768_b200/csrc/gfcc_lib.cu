@@ -64,7 +64,7 @@ struct gfcc_ctx {
   int oz_ws_nrhs = 0, oz_ws_ni = 0;
   double st_oz_gemms = 0;
   // ---- options / stats ----
-  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3e9, opt_max_batch = 256, opt_overlap = 0;
+  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3.2e9, opt_max_batch = 256, opt_overlap = 0;
   double st_iterations = 0, st_sigma_apps = 0, st_flops_sigma = 0, st_flops_create = 0, st_max_relres = 0, st_nunconv = 0;
   double st_gemm_launches = 0, st_kernel_launches = 0, st_flops_exec = 0;
   std::vector<double> last_relres;

@@ -77,7 +77,7 @@ def main():
     if a.sigma_shapes:
         o, v, Q, nrhs = SHAPES[a.sigma_shapes]
         ov, ld, Nc = o * v, o * 2 * nrhs, 2 * nrhs
-        ni = max(1, min(o, int(3e9 // (ov * 8 * v))))
+        ni = max(1, min(o, int(3.2e9 // (ov * 8 * v))))
         shapes = [("S1  Y = Lov XU", Q, ld, ov, False, False), ("S7  Z = Lm^T Y", ov, ld, Q, True, False),
                   ("S8  K2 panel build", ni * o, v * v, Q, True, False), ("S9  Z -= K2 XU (panel)", ni * v, ld, ov, False, False),
                   ("S6  W_mnij x2", o * (o - 1) // 2, v * Nc, o * (o - 1) // 2, False, False)]
