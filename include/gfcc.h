@@ -95,7 +95,12 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *   "overlap"      1: the K2 chain, the K4 chain and the small sigma terms run on three streams so that
  *                  CTAs of one chain fill the ragged last wave of another; 0 (default): everything on the handle's stream
  *   "profile_gemm" 1: bracket every GEMM-engine launch with CUDA events on the handle's stream (statistics
- *                  "gemm_time_ms", "gemm_flops_timed", "gemm_launches_timed"; implies overlap = 0 while it is on); 0: off (default) */
+ *                  "gemm_time_ms", "gemm_flops_timed", "gemm_launches_timed"; implies overlap = 0 while it is on); 0: off (default)
+ *   "engine"       0 (default): every contraction on the FP64 tensor-core (DMMA) engine; 1: S6 and S8-S11 on the INT8 tensor pipe
+ *                  with FP64 accuracy (gfcc_dgemm_ozaki's scheme; needs ~22 GB more device memory at config 4), the rest on DMMA
+ *   "ozaki_slices" digit slices of the INT8 engine, 2..8 (default 7: ~1e-13 per contraction; 6: ~1e-11)
+ * Statistics of the INT8 engine: "oz_gemms" (launches), "oz_fail" (1 if a bounded pipeline wait ever timed out; the call that
+ * notices it returns GFCC_ECUDA), "oz_time_ms" / "oz_ops_timed" / "oz_flops_timed" / "oz_launches_timed" (with profile_gemm). */
 int gfcc_set_option(gfcc_handle h, const char* key, double val);
 
 /* Statistics of the last call (double-valued): "iterations" (Arnoldi steps of the last solve),
