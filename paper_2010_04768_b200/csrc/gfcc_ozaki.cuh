@@ -735,7 +735,14 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     const char* e = getenv("GFCC_OZ_GROUP_M");
     if (e && atoi(e) > 0) p.group_m = std::min(p.tiles_m, atoi(e));
   }
-  const int grid = std::min(p.tiles_m * p.tiles_n, num_sms);
+  // persistent grid: one CTA per SM of THIS device (the producer rendezvous needs every CTA of the grid to be resident)
+  static int dev_sms = 0;
+  if (dev_sms == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) dev_sms = n;
+    else dev_sms = num_sms;
+  }
+  const int grid = std::min(p.tiles_m * p.tiles_n, std::min(num_sms, dev_sms));
   if (grid < 1) return cudaSuccess;
   {
     long long spt = 0;
