@@ -193,13 +193,20 @@ def gfcc_sigma_ip(h, omega, eta, X1, X2, S1=None, S2=None):
     return S1, S2
 
 
-def gfcc_sigma_ip_host(h, omega, eta, X1, X2):
-    """Same with HOST numpy complex128 arrays (or pinned CPU tensors); copies are inside the call."""
+def gfcc_sigma_ip_host(h, omega, eta, X1, X2, out=None):
+    """Same with HOST numpy complex128 arrays (or pinned CPU tensors); copies are inside the call.  out = (S1, S2): optional
+    preallocated host outputs of the same shapes (e.g. views of pinned tensors: the device-to-host copy then runs at full speed)."""
     X1 = np.ascontiguousarray(X1.numpy() if hasattr(X1, "numpy") else X1, dtype=np.complex128)
     X2 = np.ascontiguousarray(X2.numpy() if hasattr(X2, "numpy") else X2, dtype=np.complex128)
     nrhs = X1.shape[0]
-    S1 = np.empty_like(X1)
-    S2 = np.empty_like(X2)
+    if out is not None:
+        S1, S2 = (t.numpy() if hasattr(t, "numpy") else t for t in out)
+        if (S1.shape != X1.shape or S2.shape != X2.shape or S1.dtype != np.complex128 or S2.dtype != np.complex128
+                or not S1.flags.c_contiguous or not S2.flags.c_contiguous):
+            raise GfccError(GFCC_EINVAL, "gfcc_sigma_ip_host: out must be contiguous complex128 arrays shaped like X1, X2")
+    else:
+        S1 = np.empty_like(X1)
+        S2 = np.empty_like(X2)
     om, omp = _omega(omega, nrhs)
     _check(h, lib().gfcc_sigma_ip_host(h.ptr, nrhs, omp, float(eta), X1.ctypes.data, X2.ctypes.data, S1.ctypes.data, S2.ctypes.data))
     return S1, S2

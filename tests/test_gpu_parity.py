@@ -77,6 +77,13 @@ def test_create_and_sigma_small(o, v, Q, sym, nrhs):
     # host-buffer entry point gives the same bits
     H1, H2 = g.gfcc_sigma_ip_host(h, w, 0.01, x1, x2)
     assert np.array_equal(H1, G1.cpu().numpy()) and np.array_equal(H2, G2n)
+    # ... also into caller-provided (pinned) host outputs
+    P1 = torch.empty(x1.shape, dtype=torch.complex128, pin_memory=True)
+    P2 = torch.empty(x2.shape, dtype=torch.complex128, pin_memory=True)
+    g.gfcc_sigma_ip_host(h, w, 0.01, x1, x2, out=(P1, P2))
+    assert np.array_equal(P1.numpy(), H1) and np.array_equal(P2.numpy(), H2)
+    with pytest.raises(g.GfccError):
+        g.gfcc_sigma_ip_host(h, w, 0.01, x1, x2, out=(P2, P1))
     # exact shift identity on the GPU path too
     T1, T2 = g.gfcc_sigma_ip(h, w + 0.25, 0.01, dev(x1), dev(x2))
     assert relmax((T2 - G2).cpu().numpy(), 0.25 * x2) < 1e-12
