@@ -88,10 +88,19 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
 /* Options (double-valued):
  *   "gmres_m"      restart length (default 50; clipped to what device memory allows)
  *   "gmres_maxit"  maximum number of sigma applications per solve (default 1000)
- *   "gmres_fixed"  if > 0: run exactly this many Arnoldi steps in ONE cycle, no stop test (timing mode)
+ *   "gmres_fixed"  if > 0: run exactly this many Arnoldi steps in ONE cycle, no stop test, no compaction (timing mode);
+ *                  takes effect on every call (a later smaller value is honoured without reallocation)
  *   "x0"           0: zero initial guess, 1: zeroth-order guess b/(omega - i eta + d) (default 1)
  *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3.2e9: 5 occupied indices per panel at config 4)
  *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256)
+ *   "compact"      converged-RHS compaction (iteration counts differ between (omega,p) tasks): when at least
+ *                  max(1, compact * active columns) right-hand sides of the batch have met the stop test they are finalised and
+ *                  dropped from every live vector, so the GEMM N dimension of the following sigma applications shrinks; free
+ *                  columns are refilled from the pending (p,omega) list at the next restart boundary.  Default 0.125; < 0: never
+ *                  (lock-step batch with a done mask; same G)
+ *   "release_workspace"  (any value) free the per-batch sigma workspace and the GMRES basis now; they are re-allocated on demand
+ *   "gmres_poll"   the done flags live on the device; the host reads them every gmres_poll Arnoldi steps (0 = default: every step
+ *                  when one sigma application is >= 5 GFLOP, else every 4th step)
  *   "overlap"      1: the K2 chain, the K4 chain and the small sigma terms run on three streams so that
  *                  CTAs of one chain fill the ragged last wave of another; 0 (default): everything on the handle's stream
  *   "profile_gemm" 1: bracket every GEMM-engine launch with CUDA events on the handle's stream (statistics
@@ -106,10 +115,27 @@ int gfcc_set_option(gfcc_handle h, const char* key, double val);
 /* Statistics of the last call (double-valued): "iterations" (Arnoldi steps of the last solve),
  * "sigma_applications", "flops_sigma" (executed FP64 flop model of ONE batched application),
  * "flops_create", "bytes_device" (device memory owned by the handle), "max_relres", "n_unconverged",
- * "gemm_launches", "kernel_launches" (since create or the last reset by reading "reset_counters"). */
+ * "gemm_launches", "kernel_launches" (since create or the last reset by reading "reset_counters"),
+ * "gmres_m_used" (active restart length of the last solve), "gmres_m_cap" (allocated basis length), "gmres_m_memory_limit"
+ * (largest basis the free device memory would allow for the current batch width),
+ * "compactions", "refills", "polls", "active_col_steps" (sum over sigma applications of the last solve of the number of
+ * right-hand-side columns in the batch) and "lockstep_col_steps" (the same sum had every column stayed until its cycle ended). */
 int gfcc_get_stat(gfcc_handle h, const char* key, double* val);
 /* per right-hand-side results of the last solve: relres [host][n], iters [host][n], n = np*nw.        */
 int gfcc_get_residuals(gfcc_handle h, int n, double* relres, int* iters);
+
+/* relative residual |rotated residual| / ||b|| of right-hand side `rhs` (r = ip*nw + iw) of the last solve after each of
+ * its sigma applications: hist[0] = ||b - A x0|| / ||b||, hist[k] after Arnoldi step k (a restart contributes the true residual
+ * of its first application).  *n_out [host, nullable] = number of entries available (at most 8192 are kept); the first
+ * min(cap, n) are copied to hist [host].  When the solve had more right-hand sides than "max_batch", histories are kept for the
+ * tasks that were the last occupants of their batch column.                                                              */
+int gfcc_get_residual_history(gfcc_handle h, int rhs, int cap, double* hist, int* n_out);
+
+/* G assembly alone (first, IP term of Eq. 7-8) for caller-provided vectors:
+ *   Gout[r][iq] = <Phi|(1+Lambda1+Lambda2) abar_{q[iq]}^+ (X1_r + X2_r)|Phi> = c_q . X_r   complex [nrhs][nq]
+ * X1 [nrhs][o], X2 [nrhs][o][o][v] device, layouts of gfcc_sigma_ip (only the i<j half of X2 is read); q [host][nq] in [0,N);
+ * Gout host or device.  Linear in X: gfcc_solve_ip's G is this map applied to the solutions.  Synchronous.             */
+int gfcc_assemble_g(gfcc_handle h, int nrhs, const void* X1, const void* X2, int nq, const int* q, void* Gout);
 
 /* Copy a named intermediate to a caller buffer (device pointer, FP64), for parity tests:
  *   "Fme" [o][v], "Fmi" [o][o], "Fae" [v][v], "Wmnij" packed [npair(i<j)][npair(m<n)],

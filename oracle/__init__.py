@@ -44,6 +44,8 @@ def lib():
         L.orc_gmres.restype = ctypes.c_int
         L.orc_gmres.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                 ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_double_p, _c_double_p, _c_double_p]
+        L.orc_gmres_hist.restype = ctypes.c_int
+        L.orc_gmres_hist.argtypes = L.orc_gmres.argtypes + [_c_double_p, ctypes.c_int]
         L.orc_sigma_rows.argtypes = [ctypes.c_void_p, ctypes.c_int, _c_double_p, ctypes.c_double, _c_double_p,
                                      _c_double_p, ctypes.c_int, _c_int_p, _c_double_p, ctypes.c_int, _c_int_p,
                                      _c_double_p]
@@ -165,15 +167,19 @@ class Oracle:
         return x1, x2
 
     # ---- solves --------------------------------------------------------------------------
-    def gmres(self, p, omega, eta, tol, m=50, maxit=1000, x0kind=1):
-        """GMRES(m) for one (p, omega). Returns (x1, x2, n_sigma_applications, relres)."""
+    def gmres(self, p, omega, eta, tol, m=50, maxit=1000, x0kind=1, history=False):
+        """GMRES(m) for one (p, omega). Returns (x1, x2, n_sigma_applications, relres[, hist]); hist[k] = relative residual
+        (estimate) after sigma application k+1."""
         x1 = np.empty(self.o, dtype=np.complex128)
         x2 = np.empty((self.o, self.o, self.v), dtype=np.complex128)
         rr = np.empty(1)
-        n = lib().orc_gmres(self.h, int(p), float(omega), float(eta), float(tol), int(m), int(maxit), int(x0kind),
-                            _dp(x1.view(np.float64)), _dp(x2.view(np.float64)), _dp(rr))
+        hist = np.full(int(maxit) + 1, np.nan)
+        n = lib().orc_gmres_hist(self.h, int(p), float(omega), float(eta), float(tol), int(m), int(maxit), int(x0kind),
+                                 _dp(x1.view(np.float64)), _dp(x2.view(np.float64)), _dp(rr), _dp(hist), len(hist))
         if n < 0:
             raise RuntimeError("orc_gmres needs MODE_DEF")
+        if history:
+            return x1, x2, n, rr[0], hist[:n]
         return x1, x2, n, rr[0]
 
     def dense_hbar(self):

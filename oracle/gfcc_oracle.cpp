@@ -543,9 +543,11 @@ void orc_bra_dot(void* h, const double* c1, const double* c2, const cd* x1, cons
 // d_i = -f_ii, d_ija = f_aa - f_ii - f_jj (zeroth order; reading 11).
 // Works on the packed vector z = (x1[i], x2[i<j,a]); sigma is applied through sigma_def_one.
 // Returns the number of sigma applications; relres = final |g| / ||b||.
+// hist (nullable, nhist entries): hist[k] = the residual estimate after sigma application k+1, i.e. ||b - A x|| / ||b|| for the
+// application that starts a cycle and |g_{j+1}| / ||b|| for an Arnoldi step (an output only; the iteration does not read it).
 // ------------------------------------------------------------------------------------
-int orc_gmres(void* h, int p, double omega, double eta, double tol, int m, int maxit, int x0kind, cd* x1out,
-              cd* x2out, double* relres) {
+int orc_gmres_hist(void* h, int p, double omega, double eta, double tol, int m, int maxit, int x0kind, cd* x1out,
+                   cd* x2out, double* relres, double* hist, int nhist) {
   Ctx& c = *(Ctx*)h;
   if (!c.has_def) return -1;
   const int o = c.o, v = c.v, N = c.N;
@@ -605,6 +607,7 @@ int orc_gmres(void* h, int p, double omega, double eta, double tol, int m, int m
     for (i64 k = 0; k < n; ++k) r[k] = b[k] - w[k];
     const double beta = std::sqrt(std::real(dot(r, r)));
     res = beta / bnorm;
+    if (hist && napply - 1 < nhist) hist[napply - 1] = res;
     if (res <= tol) break;
     std::vector<std::vector<cd>> V(1, r);
     for (auto& e : V[0]) e /= beta;
@@ -635,6 +638,7 @@ int orc_gmres(void* h, int p, double omega, double eta, double tol, int m, int m
         g[j] = std::conj(cs[j]) * g[j];
       }
       res = std::abs(g[j + 1]) / bnorm;
+      if (hist && napply - 1 < nhist) hist[napply - 1] = res;
       if (res <= tol || hn == 0.0) { ++j; break; }
       V.push_back(w);
       for (auto& e : V.back()) e /= hn;
@@ -653,6 +657,11 @@ int orc_gmres(void* h, int p, double omega, double eta, double tol, int m, int m
   unpack(x, x1out, x2out);
   *relres = res;
   return napply;
+}
+
+int orc_gmres(void* h, int p, double omega, double eta, double tol, int m, int maxit, int x0kind, cd* x1out,
+              cd* x2out, double* relres) {
+  return orc_gmres_hist(h, p, omega, eta, tol, m, maxit, x0kind, x1out, x2out, relres, nullptr, 0);
 }
 
 // ------------------------------------------------------------------------------------

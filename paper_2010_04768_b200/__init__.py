@@ -22,7 +22,8 @@ LIB_PATH = os.path.join(_HERE, "libgfcc_b200.so")
 GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 
 EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
-           "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_intermediate", "gfcc_last_error",
+           "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_residual_history", "gfcc_assemble_g",
+           "gfcc_get_intermediate", "gfcc_last_error",
            "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
            "gfcc_mor_get", "gfcc_spectral_adaptive"]
 
@@ -56,6 +57,8 @@ def lib():
     L.gfcc_set_option.argtypes = [vp, ctypes.c_char_p, cd]
     L.gfcc_get_stat.argtypes = [vp, ctypes.c_char_p, dp]
     L.gfcc_get_residuals.argtypes = [vp, ci, dp, ip]
+    L.gfcc_get_residual_history.argtypes = [vp, ci, ci, dp, ip]
+    L.gfcc_assemble_g.argtypes = [vp, ci, vp, vp, ci, ip, vp]
     L.gfcc_get_intermediate.argtypes = [vp, ctypes.c_char_p, vp]
     L.gfcc_get_intermediate.restype = cll
     L.gfcc_last_error.argtypes = [vp]
@@ -158,6 +161,30 @@ def gfcc_get_residuals(h, n):
     _check(h, lib().gfcc_get_residuals(h.ptr, n, rel.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
                                        its.ctypes.data_as(ctypes.POINTER(ctypes.c_int))))
     return rel, its
+
+
+def gfcc_get_residual_history(h, rhs):
+    """relative residual of right-hand side `rhs` of the last solve after each of its sigma applications (numpy array)."""
+    n = ctypes.c_int(0)
+    _check(h, lib().gfcc_get_residual_history(h.ptr, int(rhs), 0, None, ctypes.byref(n)))
+    out = np.empty(n.value, dtype=np.float64)
+    if n.value:
+        _check(h, lib().gfcc_get_residual_history(h.ptr, int(rhs), n.value, out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                                  ctypes.byref(n)))
+    return out
+
+
+def gfcc_assemble_g(h, X1, X2, q):
+    """G assembly alone: X1 [nrhs,o], X2 [nrhs,o,o,v] complex128 CUDA tensors, q host ints -> G [nrhs, nq] numpy complex128."""
+    torch = _torch()
+    qa = np.ascontiguousarray(q, dtype=np.int32)
+    nrhs = X1.shape[0]
+    if X1.numel() != nrhs * h.o or X2.numel() != nrhs * h.o * h.o * h.v:
+        raise GfccError(GFCC_EINVAL, "X1/X2 shape mismatch")
+    G = np.empty((nrhs, len(qa)), dtype=np.complex128)
+    _check(h, lib().gfcc_assemble_g(h.ptr, nrhs, _dev(X1, torch.complex128), _dev(X2, torch.complex128), len(qa),
+                                    qa.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), G.ctypes.data))
+    return G
 
 
 def gfcc_get_intermediate(h, name):

@@ -1,8 +1,8 @@
 // =====================================================================================
-// gfcc_gemm_ws.cuh -- warp-specialised variant of the FP64 DMMA GEMM engine (sm_100a).
+// gfcc_gemm_ws.cuh -- the warp-specialised kernel of the FP64 DMMA GEMM engine (sm_100a).
 //
-// Same contraction, operand addressing and tile shapes as dgemm_dmma_kernel (gfcc_gemm.cuh; SURVEY.md 8a
-// S1,S6-S11, Eq. 11), different pipeline:
+// Contraction, operand addressing and tile shapes as described in gfcc_gemm.cuh (SURVEY.md 8a
+// S1,S6-S11, Eq. 11); pipeline:
 //   * one PRODUCER warpgroup (4 warps) does nothing but address arithmetic + cp.async (LDGSTS) into a
 //     WS_STAGES-deep ring of padded shared-memory tiles and signals "full" mbarriers through
 //     cp.async.mbarrier.arrive (completion of the copies, not their issue);

@@ -293,15 +293,17 @@ __global__ void k_abi_to_vec(double* __restrict__ vec, const double2* __restrict
     if (r < nrhs && row < n) reinterpret_cast<double2*>(vec + row * Nc)[r] = tile[threadIdx.x][rw];
   }
 }
-// vec[n][Nc] -> S1 [nrhs][o], S2 [nrhs][o][o][v] complex, antisymmetric fill, zero diagonal
+// vec[n][ld] -> S1 [.][o], S2 [.][o][o][v] complex, antisymmetric fill (the diagonal blocks are zeroed by k_zero_diag).
+// Column r of the first nrhs columns of vec goes to output vector out_row[r] (nullptr: r); ld = row stride of vec in
+// complex columns (>= nrhs).
 __global__ void k_vec_to_abi(double2* __restrict__ S1, double2* __restrict__ S2, const double* __restrict__ vec, int o, int v,
-                             int nrhs) {
+                             int nrhs, int ld = 0, const int* __restrict__ out_row = nullptr) {
   __shared__ double2 tile[32][33];
   const long long npair = (long long)o * (o - 1) / 2;
   const long long n = o + npair * v;
   const long long row0 = (long long)blockIdx.x * 32;
   const int r0 = blockIdx.y * 32;
-  const int Nc = 2 * nrhs;
+  const long long Nc = 2LL * (ld > 0 ? ld : nrhs);
   for (int rw = threadIdx.y; rw < 32; rw += blockDim.y) {
     const long long row = row0 + rw;
     const int r = r0 + threadIdx.x;
@@ -312,42 +314,62 @@ __global__ void k_vec_to_abi(double2* __restrict__ S1, double2* __restrict__ S2,
     const int r = r0 + rr;
     const long long row = row0 + threadIdx.x;
     if (r < nrhs && row < n) {
+      const long long ro = out_row ? out_row[r] : r;
       const double2 val = tile[rr][threadIdx.x];
-      if (row < o) S1[(long long)r * o + row] = val;
+      if (row < o) S1[ro * o + row] = val;
       else {
         const long long q = row - o;
         const long long pr = q / v;
         const int a = q % v;
         int i, j;
         decode_pair(pr, o, i, j);
-        S2[(((long long)r * o + i) * o + j) * v + a] = val;
-        S2[(((long long)r * o + j) * o + i) * v + a] = make_double2(-val.x, -val.y);
+        S2[((ro * o + i) * o + j) * v + a] = val;
+        S2[((ro * o + j) * o + i) * v + a] = make_double2(-val.x, -val.y);
       }
     }
   }
 }
-__global__ void k_zero_diag(double2* __restrict__ S2, int o, int v, int nrhs) {
+// zero the i == j blocks of output vectors out_row[r] (nullptr: r), r < nrhs
+__global__ void k_zero_diag(double2* __restrict__ S2, int o, int v, int nrhs, const int* __restrict__ out_row = nullptr) {
   const long long total = (long long)nrhs * o * v;
   for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
     const int a = idx % v;
     const int i = (idx / v) % o;
     const int r = idx / ((long long)v * o);
-    S2[(((long long)r * o + i) * o + i) * v + a] = make_double2(0.0, 0.0);
+    const long long ro = out_row ? out_row[r] : r;
+    S2[((ro * o + i) * o + i) * v + a] = make_double2(0.0, 0.0);
   }
 }
 
-// XU[m][e][j][c] = x2[m,j,e,c]   from the packed vector (rows o + pair*v + e), antisymmetric fill
-__global__ void k_unpack_xu(double* __restrict__ XU, const double* __restrict__ vec, int o, int v, int Nc) {
-  // grid: (m*v + e) in blockIdx.x ; threads over (j, c)
+// XU[m][e][j][c] = x2[m,j,e,c]   from the packed vector (rows o + pair*v + e), antisymmetric fill.
+// One block per (m, e): the destination row (o*Nc doubles) is contiguous; the sources are Nc-double pieces, one per j.
+// 16-byte accesses (Nc is even), four independent loads in flight per thread.
+__global__ void __launch_bounds__(256) k_unpack_xu(double* __restrict__ XU, const double* __restrict__ vec, int o, int v, int Nc) {
   const int m = blockIdx.x / v, e = blockIdx.x % v;
-  double* dst = XU + (long long)blockIdx.x * o * Nc;
-  const double* x2 = vec + (long long)o * Nc;
-  for (int t = threadIdx.x; t < o * Nc; t += blockDim.x) {
-    const int j = t / Nc, c = t % Nc;
-    double val = 0.0;
-    if (m < j) val = x2[(pair_index(m, j, o) * v + e) * Nc + c];
-    else if (m > j) val = -x2[(pair_index(j, m, o) * v + e) * Nc + c];
-    dst[t] = val;
+  const int nr = Nc >> 1;                                             // complex columns
+  double2* __restrict__ dst = reinterpret_cast<double2*>(XU + (long long)blockIdx.x * o * Nc);
+  const double2* __restrict__ x2 = reinterpret_cast<const double2*>(vec + (long long)o * Nc);
+  const int total = o * nr;
+  for (int t0 = threadIdx.x; t0 < total; t0 += 4 * blockDim.x) {
+    double2 val[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int t = t0 + u * blockDim.x;
+      val[u] = make_double2(0.0, 0.0);
+      if (t < total) {
+        const int j = t / nr, c = t - j * nr;
+        if (m < j) val[u] = x2[(pair_index(m, j, o) * v + e) * nr + c];
+        else if (m > j) {
+          const double2 q = x2[(pair_index(j, m, o) * v + e) * nr + c];
+          val[u] = make_double2(-q.x, -q.y);
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int t = t0 + u * blockDim.x;
+      if (t < total) dst[t] = val[u];
+    }
   }
 }
 
@@ -395,31 +417,51 @@ __global__ void k_sigma1_small(double* __restrict__ sout, const double* __restri
 }
 
 // sigma2 epilogue: s2[(i<j)][a][c] += (w - i eta) x2 + Z[i][a][j][c] - Z[j][a][i][c]
-__global__ void k_sigma2_epilogue(double* __restrict__ sout, const double* __restrict__ xin, const double* __restrict__ Z,
-                                  const double* __restrict__ omega, double eta, int o, int v, int nrhs) {
-  // blockIdx.x = pair*v + a ; threads over r
-  const long long row = blockIdx.x;
-  const long long pr = row / v;
-  const int a = row % v;
+// One block per pair (i<j): the pair is decoded once; the block's rows of x2 / s2 (v*Nc doubles) are contiguous, the two Z
+// operands come as Nc-double pieces (one per a).  One thread per complex element, four elements (16 independent 16-byte
+// loads) in flight per thread.
+__global__ void __launch_bounds__(256) k_sigma2_epilogue(double* __restrict__ sout, const double* __restrict__ xin,
+                                                         const double* __restrict__ Z, const double* __restrict__ omega, double eta,
+                                                         int o, int v, int nrhs) {
+  const long long pr = blockIdx.x;
   int i, j;
   decode_pair(pr, o, i, j);
-  const int Nc = 2 * nrhs;
-  const double2* x = reinterpret_cast<const double2*>(xin + ((long long)o + row) * Nc);
-  double2* s = reinterpret_cast<double2*>(sout + ((long long)o + row) * Nc);
-  const double2* zij = reinterpret_cast<const double2*>(Z + (((long long)i * v + a) * o + j) * Nc);
-  const double2* zji = reinterpret_cast<const double2*>(Z + (((long long)j * v + a) * o + i) * Nc);
-  for (int r = threadIdx.x; r < nrhs; r += blockDim.x) {
-    const double w = omega[r];
-    const double2 xv = x[r], p = zij[r], q = zji[r];
-    double2 cur = s[r];
-    cur.x += w * xv.x + eta * xv.y + p.x - q.x;
-    cur.y += w * xv.y - eta * xv.x + p.y - q.y;
-    s[r] = cur;
+  const long long row0 = (long long)o + pr * v;
+  const double2* __restrict__ x = reinterpret_cast<const double2*>(xin) + row0 * nrhs;
+  double2* __restrict__ s = reinterpret_cast<double2*>(sout) + row0 * nrhs;
+  const double2* __restrict__ zij = reinterpret_cast<const double2*>(Z) + ((long long)i * v * o + j) * nrhs;   // + a*o*nrhs + r
+  const double2* __restrict__ zji = reinterpret_cast<const double2*>(Z) + ((long long)j * v * o + i) * nrhs;
+  const long long za = (long long)o * nrhs;
+  const int total = v * nrhs;
+  for (int t0 = threadIdx.x; t0 < total; t0 += 4 * blockDim.x) {
+    double2 xv[4], cur[4], p[4], q[4];
+    double w[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int t = t0 + u * blockDim.x;
+      if (t < total) {
+        const int a = t / nrhs, r = t - a * nrhs;
+        xv[u] = x[t]; cur[u] = s[t]; p[u] = zij[a * za + r]; q[u] = zji[a * za + r]; w[u] = omega[r];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int t = t0 + u * blockDim.x;
+      if (t < total) {
+        cur[u].x += w[u] * xv[u].x + eta * xv[u].y + p[u].x - q[u].x;
+        cur[u].y += w[u] * xv[u].y - eta * xv[u].x + p[u].y - q[u].y;
+        s[t] = cur[u];
+      }
+    }
   }
 }
 
 // ------------------------------------------------------------------------------------
-// GMRES building blocks on vec[n][Nc] matrices (complex columns = double2 per rhs)
+// GMRES building blocks on vec[n][Nc] matrices (complex columns = double2 per active right-hand side).
+// Vectors are indexed by the ACTIVE column r in [0, nrhs) (compact layout, row stride nrhs complex numbers); the small
+// per-RHS arrays of the solver (Hessenberg columns, rotations, scales, flags) are indexed by the SLOT the right-hand side
+// occupies for its whole life in the batch: element (k, r) lives at [k*ldc + slot[r]] (slot == nullptr: slot[r] = r), so
+// that dropping converged columns from the vectors (gfcc_solve.cuh) never moves the small arrays.
 // ------------------------------------------------------------------------------------
 // partial[blk][k][r] = sum over this block's rows of conj(V_k[row][r]) * w[row][r],  k in [0,nk), nk <= NK.
 // blockDim = (TX rhs lanes, TY row lanes); gridDim = (row blocks, ceil(nrhs/TX)); dynamic smem TX*TY double2.
@@ -465,9 +507,9 @@ __global__ void k_multi_dot(double2* __restrict__ partial, const double* const* 
     }
   }
 }
-// h[k][r] (+)= sum_blk partial[blk][k][r]
+// h[k*ldc + slot[r]] (+)= sum_blk partial[blk][k][r]
 __global__ void k_dot_finish(double2* __restrict__ h, const double2* __restrict__ partial, int nblk, int nk, int nrhs,
-                             int accumulate) {
+                             int accumulate, const int* __restrict__ slot, int ldc) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= nk * nrhs) return;
   double2 s = make_double2(0.0, 0.0);
@@ -476,22 +518,25 @@ __global__ void k_dot_finish(double2* __restrict__ h, const double2* __restrict_
     s.x += t.x;
     s.y += t.y;
   }
-  if (accumulate) { s.x += h[idx].x; s.y += h[idx].y; }
-  h[idx] = s;
+  const int k = idx / nrhs, r = idx - k * nrhs;
+  const long long out = (long long)k * ldc + (slot ? slot[r] : r);
+  if (accumulate) { s.x += h[out].x; s.y += h[out].y; }
+  h[out] = s;
 }
-// w[row][r] += sign * sum_k coef[k][r] * V_k[row][r]     (nk <= NK per launch)
+// w[row][r] += sign * sum_k coef[k*ldc + slot[r]] * V_k[row][r]     (nk <= NK per launch)
 template <int NK>
 __global__ void k_multi_axpy(double* __restrict__ w, const double* const* __restrict__ Vs, const double2* __restrict__ coef,
-                             long long n, int nrhs, int nk, double sign) {
+                             long long n, int nrhs, int nk, double sign, const int* __restrict__ slot, int ldc) {
   const long long total = n * nrhs;
   for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
     const long long row = idx / nrhs;
     const int r = idx % nrhs;
+    const int sl = slot ? slot[r] : r;
     double2 acc = reinterpret_cast<double2*>(w)[idx];
 #pragma unroll
     for (int k = 0; k < NK; ++k)
       if (k < nk) {
-        const double2 c = coef[(long long)k * nrhs + r];
+        const double2 c = coef[(long long)k * ldc + sl];
         const double2 vv = reinterpret_cast<const double2*>(Vs[k])[row * nrhs + r];
         acc.x += sign * (c.x * vv.x - c.y * vv.y);
         acc.y += sign * (c.x * vv.y + c.y * vv.x);
@@ -499,28 +544,44 @@ __global__ void k_multi_axpy(double* __restrict__ w, const double* const* __rest
     reinterpret_cast<double2*>(w)[idx] = acc;
   }
 }
-// out[row][r] = scale[r] * in[row][r]   (real scale per rhs; scale 0 masks a converged / broken-down column)
+// out[row][r] = scale[slot[r]] * in[row][r]   (real scale per rhs; scale 0 masks a converged / broken-down column)
 __global__ void k_scale_cols(double* __restrict__ out, const double* __restrict__ in, const double* __restrict__ scale,
-                             long long n, int nrhs) {
+                             long long n, int nrhs, const int* __restrict__ slot) {
   const long long total = n * nrhs;
   for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
     const int r = idx % nrhs;
-    const double s = scale[r];
+    const double s = scale[slot ? slot[r] : r];
     double2 x = reinterpret_cast<const double2*>(in)[idx];
     x.x *= s;
     x.y *= s;
     reinterpret_cast<double2*>(out)[idx] = x;
   }
 }
-// a[k] += b[k] (complex arrays)
-__global__ void k_cadd(double2* __restrict__ a, const double2* __restrict__ b, int n) {
+// a[k*ldc + slot[r]] += b[k*ldc + slot[r]] for k < nk, r < nrhs (complex arrays)
+__global__ void k_cadd(double2* __restrict__ a, const double2* __restrict__ b, int nk, int nrhs, const int* __restrict__ slot, int ldc) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx < n) { a[idx].x += b[idx].x; a[idx].y += b[idx].y; }
+  if (idx >= nk * nrhs) return;
+  const int k = idx / nrhs, r = idx - k * nrhs;
+  const long long q = (long long)k * ldc + (slot ? slot[r] : r);
+  a[q].x += b[q].x; a[q].y += b[q].y;
 }
 // r = b - Ax
 __global__ void k_residual(double* __restrict__ r, const double* __restrict__ b, const double* __restrict__ ax, long long n2) {
   for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n2; idx += (long long)gridDim.x * blockDim.x)
     r[idx] = b[idx] - ax[idx];
+}
+// column gather between two batch layouts (converged-RHS compaction, refill, retirement; gfcc_solve.cuh):
+//   dst[row][dcol0 + c] = src[row][src_col[c]]  for c < ncopy  (src_col[c] < 0: zero);  row strides ldd / lds complex columns
+__global__ void k_gather_cols(double* __restrict__ dst, int ldd, int dcol0, const double* __restrict__ src, int lds,
+                              const int* __restrict__ src_col, int ncopy, long long n) {
+  const long long total = n * ncopy;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const long long row = idx / ncopy;
+    const int c = idx - row * ncopy;
+    const int sc = src_col[c];
+    reinterpret_cast<double2*>(dst)[row * ldd + dcol0 + c] =
+        sc >= 0 ? reinterpret_cast<const double2*>(src)[row * lds + sc] : make_double2(0.0, 0.0);
+  }
 }
 
 }  // namespace gfcc

@@ -65,10 +65,12 @@ struct gfcc_ctx {
   double st_oz_gemms = 0;
   // ---- options / stats ----
   double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3.2e9, opt_max_batch = 256, opt_overlap = 0;
+  double opt_compact = 0.125, opt_poll = 0;
   double st_iterations = 0, st_sigma_apps = 0, st_flops_sigma = 0, st_flops_create = 0, st_max_relres = 0, st_nunconv = 0;
   double st_gemm_launches = 0, st_kernel_launches = 0, st_flops_exec = 0;
   std::vector<double> last_relres;
   std::vector<int> last_iters;
+  std::vector<std::vector<double>> last_hist;   // per right-hand side: relative residual after every sigma application
   SolveWs sw;
   // ---- MOR subspace: S, Hbar*S as [n_pad][cap] real, H^ as [cap][cap] ----
   int mor_cap = 0, mor_m = 0;
@@ -216,25 +218,37 @@ static int choose_panel(int o, int v, long long ncols, double budget_bytes) {
   return best;
 }
 
+// The workspace holds room for ws_nrhs right-hand sides and serves every batch of at most that many (the solver shrinks
+// its batch when right-hand sides converge).  ws_nrhs is committed only when every allocation has succeeded; a failed
+// allocation releases whatever the call had obtained, so the handle never keeps a half-built workspace.
 static int ensure_workspace(gfcc_ctx* h, int nrhs, bool need_abi_vecs) {
   const int o = h->o, v = h->v, Q = h->Q;
-  if (h->ws_nrhs != nrhs) {
-    if (h->ws_nrhs) free_workspace(h);
+  if (h->ws_nrhs < nrhs) {
+    if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); }
     const long long Nc = 2LL * nrhs, big = (long long)o * v * o * Nc;
     h->panel_ni = h->opt_engine == 1 ? oz_choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes)
                                      : choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes);
-    h->ws_nrhs = nrhs;
-    TRY(dev_alloc(h, &h->XU, big)); TRY(dev_alloc(h, &h->Z, big)); TRY(dev_alloc(h, &h->V, big));
-    TRY(dev_alloc(h, &h->Y, (long long)Q * o * Nc));
-    TRY(dev_alloc(h, &h->KP, (long long)h->panel_ni * v * o * v));
-    if (h->opt_overlap != 0) TRY(dev_alloc(h, &h->KP2, (long long)h->panel_ni * v * o * v));
-    TRY(dev_alloc(h, &h->yv, (long long)v * Nc));
-    TRY(dev_alloc(h, &h->d_omega, nrhs));
+    h->ws_nrhs = nrhs;   // free_workspace() sizes its bookkeeping with it; reset to 0 there if anything below fails
+    int rc = GFCC_OK;
+    do {
+      if ((rc = dev_alloc(h, &h->XU, big))) break;
+      if ((rc = dev_alloc(h, &h->Z, big))) break;
+      if ((rc = dev_alloc(h, &h->V, big))) break;
+      if ((rc = dev_alloc(h, &h->Y, (long long)Q * o * Nc))) break;
+      if ((rc = dev_alloc(h, &h->KP, (long long)h->panel_ni * v * o * v))) break;
+      if (h->opt_overlap != 0 && (rc = dev_alloc(h, &h->KP2, (long long)h->panel_ni * v * o * v))) break;
+      if ((rc = dev_alloc(h, &h->yv, (long long)v * Nc))) break;
+      if ((rc = dev_alloc(h, &h->d_omega, nrhs))) break;
+    } while (0);
+    if (rc != GFCC_OK) { free_workspace(h); return rc; }
   }
   if (need_abi_vecs && !h->vin) {
-    const long long Nc = 2LL * nrhs;
-    TRY(dev_alloc(h, &h->vin, h->nvec * Nc));
-    TRY(dev_alloc(h, &h->vout, h->nvec * Nc));
+    const long long Nc = 2LL * h->ws_nrhs;
+    double *a = nullptr, *b = nullptr;
+    int rc = dev_alloc(h, &a, h->nvec * Nc);
+    if (rc == GFCC_OK && (rc = dev_alloc(h, &b, h->nvec * Nc)) != GFCC_OK) dev_free(h, a, h->nvec * Nc);
+    if (rc != GFCC_OK) return rc;
+    h->vin = a; h->vout = b;
   }
   return GFCC_OK;
 }
@@ -397,7 +411,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     TRY(gemm(h, d));
   }
   // S13: shift + P(ij) ring
-  k_sigma2_epilogue<<<(unsigned)(h->npair * v), 64, 0, s0>>>(sout, xin, h->Z, d_omega, eta, o, v, nrhs);
+  k_sigma2_epilogue<<<(unsigned)h->npair, 256, 0, s0>>>(sout, xin, h->Z, d_omega, eta, o, v, nrhs);
   KLAUNCH(h);
   h->st_sigma_apps += 1;
   return GFCC_OK;
@@ -784,6 +798,9 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "x0" && (val == 0 || val == 1)) h->opt_x0 = val;
   else if (k == "panel_bytes" && val > 0) { h->opt_panel_bytes = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
+  else if (k == "release_workspace") { cudaStreamSynchronize(h->stream); if (h->ws_nrhs) free_workspace(h); solve_free(h->sw); }
+  else if (k == "compact" && val <= 1) h->opt_compact = val;
+  else if (k == "gmres_poll" && val >= 0) h->opt_poll = std::floor(val);
   else if (k == "overlap" && (val == 0 || val == 1)) { h->opt_overlap = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "engine" && (val == 0 || val == 1)) { h->opt_engine = (int)val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "ozaki_slices" && val >= 2 && val <= OZ_MAX_SLICES) {
@@ -818,7 +835,14 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
                        cudaMemcpy(&hf, h->oz_fail, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)) { h->err = "sync failed"; return GFCC_ECUDA; }
     *val = hf;
   }
-  else if (k == "gmres_m_used") *val = h->sw.m;
+  else if (k == "gmres_m_used") *val = h->sw.m_run;
+  else if (k == "gmres_m_cap") *val = h->sw.mcap;
+  else if (k == "gmres_m_memory_limit") *val = solve_mmax(h->nvec, std::max(1, h->sw.cap > 0 ? h->sw.cap : (int)h->opt_max_batch)) + (h->sw.cap > 0 ? h->sw.mcap + 6 : 0);
+  else if (k == "compactions") *val = (double)h->sw.compactions;
+  else if (k == "refills") *val = (double)h->sw.refills;
+  else if (k == "polls") *val = (double)h->sw.polls;
+  else if (k == "active_col_steps") *val = h->sw.active_col_steps;
+  else if (k == "lockstep_col_steps") *val = h->sw.full_col_steps;
   else if (k == "oz_time_ms" || k == "oz_ops_timed" || k == "oz_flops_timed" || k == "oz_launches_timed") {
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) { h->err = "sync failed"; return GFCC_ECUDA; }
     double ms = 0, ops = 0, fl = 0, n = 0;
@@ -974,17 +998,9 @@ extern "C" int gfcc_dgemm_ozaki(void* stream, int M, int N, int K, double alpha,
     if (oz_slice(a, sa, st) != cudaSuccess || oz_slice(b, sb, st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     cudaEventRecord(ev[1], st);
     OzCDesc c; c.C = C; c.sCm0 = sCm; c.sCn0 = sCn; c.alpha = alpha; c.beta = beta;
-    long long* dbg = nullptr;
-    if (getenv("GFCC_OZ_DEBUG")) { cudaMalloc(&dbg, 128); cudaMemsetAsync(dbg, 0, 128, st); }
-    if (oz_igemm(sa, sb, c, fail, st, 148, dbg, reinterpret_cast<unsigned*>(fail) + 1) != cudaSuccess) { rc = GFCC_ECUDA; break; }
+    if (oz_igemm(sa, sb, c, fail, st, 148, nullptr, reinterpret_cast<unsigned*>(fail) + 1) != cudaSuccess) { rc = GFCC_ECUDA; break; }
     cudaEventRecord(ev[2], st);
     if (cudaStreamSynchronize(st) != cudaSuccess) { rc = GFCC_ECUDA; break; }
-    if (dbg) {
-      long long hd[16];
-      cudaMemcpy(hd, dbg, 128, cudaMemcpyDeviceToHost); cudaFree(dbg);
-      fprintf(stderr, "oz dbg (CTA 0, cycles): producer wait empty %lld | mma wait tempty %lld, wait full %lld | epilogue wait tfull %lld, "
-              "whole epilogue %lld over %lld units\n", hd[0], hd[1], hd[2], hd[3], hd[5], hd[6]);
-    }
     int hfail = 0;
     cudaMemcpy(&hfail, fail, sizeof(int), cudaMemcpyDeviceToHost);
     if (hfail) { rc = GFCC_ECUDA; break; }
@@ -1010,26 +1026,6 @@ extern "C" int gfcc_probe_fp64_peak(void* stream, int iters, int reps, double* t
 // ------------------------------------------------------------------------------------------
 // gfcc_solve_ip : batched GMRES + G assembly (gfcc_solve.cuh holds the kernels and the driver loop)
 // ------------------------------------------------------------------------------------------
-static int solve_batch(gfcc_handle h, int nrhs, const int* p_of_rhs, const double* w_of_rhs, double eta, double tol,
-                       double2* Gq_dev /* [nrhs][nq] */, const int* qlist, int nq, double* X1out, double* X2out, int rhs_offset,
-                       int nrhs_total) {
-  TRY(ensure_workspace(h, nrhs, false));
-  SolveCfg cfg;
-  cfg.o = h->o; cfg.v = h->v; cfg.nrhs = nrhs; cfg.nvec = h->nvec; cfg.npair = h->npair;
-  cfg.m = (int)h->opt_m; cfg.maxit = (int)h->opt_maxit; cfg.fixed = (int)h->opt_fixed; cfg.x0 = (int)h->opt_x0;
-  cfg.eta = eta; cfg.tol = tol;
-  cfg.t1 = h->t1; cfg.l1 = h->l1; cfg.T2p = h->T2p; cfg.L2p = h->L2p; cfg.D = h->D; cfg.fdiag = h->fdiag;
-  cfg.stream = h->stream;
-  auto apply = [&](const double* xin, double* sout) -> int { return sigma_internal(h, nrhs, h->d_omega, eta, xin, sout); };
-  std::string err;
-  double nlaunch = 0;
-  int rc = solve_run(h->sw, cfg, p_of_rhs, w_of_rhs, h->d_omega, apply, Gq_dev, qlist, nq, X1out, X2out, rhs_offset, nrhs_total,
-                     h->last_relres, h->last_iters, &h->st_iterations, &nlaunch, err);
-  h->st_kernel_launches += nlaunch;
-  if (rc == GFCC_ECUDA || rc == GFCC_ENOMEM || rc == GFCC_EINVAL) h->err = err;
-  return rc;
-}
-
 extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol,
                                void* G, void* X1out, void* X2out) {
   if (!h) return GFCC_EINVAL;
@@ -1039,30 +1035,38 @@ extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, cons
   const int ntot = np * nw;
   h->last_relres.assign(ntot, 0.0);
   h->last_iters.assign(ntot, 0);
+  h->last_hist.assign(ntot, std::vector<double>());
   h->st_iterations = 0;
-  std::vector<int> pr(ntot);
-  std::vector<double> wr(ntot);
+  std::vector<SolveTask> tasks(ntot);
   for (int ip = 0; ip < np; ++ip)
-    for (int iw = 0; iw < nw; ++iw) { pr[ip * nw + iw] = p[ip]; wr[ip * nw + iw] = omega[iw]; }
+    for (int iw = 0; iw < nw; ++iw) { tasks[ip * nw + iw].p = p[ip]; tasks[ip * nw + iw].omega = omega[iw]; }
+  const int batch = std::max(1, std::min(ntot, (int)h->opt_max_batch));
+  TRY(ensure_workspace(h, batch, false));
   double* Gq = nullptr;   // [ntot][np] complex
   TRY(dev_alloc(h, &Gq, (long long)ntot * np * 2));
   int* dq = nullptr;
-  { double* t = nullptr; TRY(dev_alloc(h, &t, np)); dq = (int*)t; }
+  { double* t = nullptr; int rc = dev_alloc(h, &t, np); if (rc) { dev_free(h, Gq, (long long)ntot * np * 2); return rc; } dq = (int*)t; }
   int rc_final = GFCC_OK;
   do {
     if (cudaMemcpyAsync(dq, p, (size_t)np * sizeof(int), cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { h->err = "H2D failed"; rc_final = GFCC_ECUDA; break; }
-    const int maxb = std::max(1, (int)h->opt_max_batch);
-    // equal-sized batches so that the workspace is allocated once
-    const int nb = (ntot + maxb - 1) / maxb;
-    const int bsz = (ntot + nb - 1) / nb;
-    for (int r0 = 0; r0 < ntot; r0 += bsz) {
-      const int n = std::min(bsz, ntot - r0);
-      int rc = solve_batch(h, n, pr.data() + r0, wr.data() + r0, eta, tol, (double2*)Gq + (long long)r0 * np, dq, np,
-                           (double*)X1out, (double*)X2out, r0, ntot);
-      if (rc == GFCC_ENOCONV) rc_final = GFCC_ENOCONV;
-      else if (rc != GFCC_OK) { rc_final = rc; break; }
-    }
-    if (rc_final != GFCC_OK && rc_final != GFCC_ENOCONV) break;
+    SolveCfg cfg;
+    cfg.o = h->o; cfg.v = h->v; cfg.nvec = h->nvec; cfg.npair = h->npair;
+    cfg.m = (int)h->opt_m; cfg.maxit = (int)h->opt_maxit; cfg.fixed = (int)h->opt_fixed; cfg.x0 = (int)h->opt_x0;
+    cfg.batch = batch; cfg.compact = h->opt_compact;
+    // polling period of the device-side done flags: every step when one sigma application is long, every 4th for tiny systems
+    cfg.poll = h->opt_poll > 0 ? (int)h->opt_poll : (sigma_flops(h, batch) < 5e9 ? 4 : 1);
+    cfg.eta = eta; cfg.tol = tol;
+    cfg.t1 = h->t1; cfg.l1 = h->l1; cfg.T2p = h->T2p; cfg.L2p = h->L2p; cfg.D = h->D; cfg.fdiag = h->fdiag;
+    cfg.stream = h->stream;
+    SigmaFn apply = [&](int nrhs, const double* d_omega, const double* xin, double* sout) -> int {
+      return sigma_internal(h, nrhs, d_omega, eta, xin, sout);
+    };
+    std::string err;
+    double nlaunch = 0;
+    int rc = solve_run(h->sw, cfg, tasks, apply, (double2*)Gq, dq, np, (double*)X1out, (double*)X2out, &h->last_hist, &nlaunch, err);
+    h->st_kernel_launches += nlaunch;
+    if (rc == GFCC_ENOCONV) rc_final = GFCC_ENOCONV;
+    else if (rc != GFCC_OK) { h->err = err; rc_final = rc; break; }
     // G[iw][ip][iq] <- Gq[(ip*nw+iw)][iq]
     std::vector<double> hostG((size_t)ntot * np * 2), outG((size_t)ntot * np * 2);
     if (cudaMemcpyAsync(hostG.data(), Gq, hostG.size() * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
@@ -1079,15 +1083,70 @@ extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, cons
   dev_free(h, (double*)dq, np);
   h->st_max_relres = 0; h->st_nunconv = 0;
   for (int k = 0; k < ntot; ++k) {
-    h->st_max_relres = std::max(h->st_max_relres, h->last_relres[k]);
-    if (h->opt_fixed == 0 && !(h->last_relres[k] <= tol)) h->st_nunconv += 1;
+    h->last_relres[k] = tasks[k].relres;
+    h->last_iters[k] = tasks[k].iters;
+    h->st_iterations = std::max(h->st_iterations, (double)tasks[k].iters);
+    h->st_max_relres = std::max(h->st_max_relres, tasks[k].relres);
+    if (h->opt_fixed == 0 && !tasks[k].converged) h->st_nunconv += 1;
   }
-  h->st_flops_sigma = sigma_flops(h, h->ws_nrhs > 0 ? h->ws_nrhs : 1);
+  h->st_flops_sigma = sigma_flops(h, batch);
   return rc_final;
 }
 
 extern "C" int gfcc_solve_ip(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol, void* G) {
   return gfcc_solve_ip_x(h, np, p, nw, omega, eta, tol, G, nullptr, nullptr);
+}
+
+// relative residual of right-hand side `rhs` of the last solve after each of its sigma applications
+extern "C" int gfcc_get_residual_history(gfcc_handle h, int rhs, int cap, double* hist, int* n_out) {
+  if (!h || rhs < 0 || (size_t)rhs >= h->last_hist.size() || cap < 0 || (cap > 0 && !hist)) return GFCC_EINVAL;
+  const std::vector<double>& v = h->last_hist[rhs];
+  if (n_out) *n_out = (int)v.size();
+  for (int k = 0; k < cap && k < (int)v.size(); ++k) hist[k] = v[k];
+  return GFCC_OK;
+}
+
+// G assembly of caller-provided vectors (first term of Eq. 7-8): Gout[r][iq] = c_{q[iq]} . X_r
+extern "C" int gfcc_assemble_g(gfcc_handle h, int nrhs, const void* X1, const void* X2, int nq, const int* q, void* Gout) {
+  if (!h) return GFCC_EINVAL;
+  if (nrhs < 1 || nq < 1 || !X1 || !X2 || !q || !Gout) { h->err = "gfcc_assemble_g: null pointer or nrhs/nq < 1"; return GFCC_EINVAL; }
+  for (int k = 0; k < nq; ++k)
+    if (q[k] < 0 || q[k] >= h->N) { h->err = "gfcc_assemble_g: orbital out of range"; return GFCC_EINVAL; }
+  const int o = h->o, v = h->v;
+  const long long Nc = 2LL * nrhs;
+  cudaStream_t st = h->stream;
+  const int g_blocks = (int)std::min<long long>(296, h->npair);
+  double *vec = nullptr, *gpart = nullptr, *gvec = nullptr, *Gq = nullptr, *dqd = nullptr;
+  int rc = GFCC_OK;
+  do {
+    if ((rc = dev_alloc(h, &vec, h->nvec * Nc))) break;
+    if ((rc = dev_alloc(h, &gpart, (long long)g_blocks * v * Nc))) break;
+    if ((rc = dev_alloc(h, &gvec, (long long)v * Nc))) break;
+    if ((rc = dev_alloc(h, &Gq, (long long)nrhs * nq * 2))) break;
+    if ((rc = dev_alloc(h, &dqd, nq))) break;
+    int* dq = (int*)dqd;
+    rc = GFCC_ECUDA;
+    if (cudaMemcpyAsync(dq, q, (size_t)nq * sizeof(int), cudaMemcpyHostToDevice, st) != cudaSuccess) { h->err = "H2D failed"; break; }
+    dim3 blk(32, 8), grid((unsigned)((h->nvec + 31) / 32), (unsigned)((nrhs + 31) / 32));
+    k_abi_to_vec<<<grid, blk, 0, st>>>(vec, (const double2*)X1, (const double2*)X2, o, v, nrhs);
+    h->st_kernel_launches += 1;
+    if (cudaFuncSetAttribute(k_lambda2_g, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) { h->err = "smem attribute"; break; }
+    dim3 lg((unsigned)((Nc + LG_CC - 1) / LG_CC), g_blocks);
+    k_lambda2_g<<<lg, 32 * LG_WARPS, lambda2_g_smem_bytes(v), st>>>(gpart, h->L2p, vec, o, v, (int)Nc, h->npair);
+    const long long n = (long long)v * Nc;
+    k_g_reduce<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(gvec, gpart, g_blocks, n);
+    dim3 gg(nq, nrhs);
+    k_assemble_G<<<gg, 256, 0, st>>>((double2*)Gq, dq, nq, vec, gvec, h->D, h->t1, h->l1, o, v, nrhs, nullptr);
+    h->st_kernel_launches += 3;
+    if (cudaGetLastError() != cudaSuccess) { h->err = "gfcc_assemble_g: launch failed"; break; }
+    if (cudaMemcpyAsync(Gout, Gq, (size_t)nrhs * nq * 16, cudaMemcpyDefault, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) { h->err = "gfcc_assemble_g: copy of G failed"; break; }
+    rc = GFCC_OK;
+  } while (0);
+  cudaStreamSynchronize(st);
+  dev_free(h, vec, h->nvec * Nc); dev_free(h, gpart, (long long)g_blocks * v * Nc); dev_free(h, gvec, (long long)v * Nc);
+  dev_free(h, Gq, (long long)nrhs * nq * 2); dev_free(h, dqd, nq);
+  return rc;
 }
 
 #include "gfcc_mor_host.inl"

@@ -108,12 +108,15 @@ __global__ void __launch_bounds__(256) k_oz_absmax(OzOperand a, unsigned long lo
   if (threadIdx.x < OZ_TR && r0 + threadIdx.x < a.R && smax[threadIdx.x] != 0ull) atomicMax(&amax[r0 + threadIdx.x], smax[threadIdx.x]);
 }
 
-// scale[r] = 2^(e-6) with max|x[r][:]| < 2^e ; 0 for a zero row.  inv[r] = 2^(6-e) is recomputed in k_oz_slice.
+// scale[r] = 2^(e-6) with max|x[r][:]| < 2^e ; 0 for a zero row; NaN for a row that holds an Inf or a NaN (its digits are
+// zero and the epilogue's scale product turns the whole output row / column into NaN, as an FP64 GEMM would).
+// inv[r] = 2^(6-e) is recomputed in k_oz_slice.
 __global__ void k_oz_exponent(const unsigned long long* __restrict__ amax, double* __restrict__ scale, int R) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= R) return;
   const double m = __longlong_as_double((long long)amax[r]);
-  if (!(m > 0.0) || !isfinite(m)) { scale[r] = 0.0; return; }
+  if (!isfinite(m)) { scale[r] = __longlong_as_double(0x7ff8000000000000ll); return; }
+  if (!(m > 0.0)) { scale[r] = 0.0; return; }
   int e;
   frexp(m, &e);                       // m = f * 2^e, f in [0.5, 1)  =>  |x| <= m < 2^e
   scale[r] = ldexp(1.0, e - 6);
@@ -669,11 +672,7 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     attr = true;
   }
   // short K: the register-accumulating 128 x 128 kernel (C written once); long K: 128 x 256 tiles with per-unit read-modify-write
-  bool regacc = A.K <= 16384;     // (<= 8 entries per accumulator x K x 64^2 stays far below 2^31)
-  {
-    const char* e = getenv("GFCC_OZ_REGACC");
-    if (e) regacc = atoi(e) != 0 && A.Kpad <= 65536;
-  }
+  const bool regacc = A.K <= 16384;     // (<= 8 entries per accumulator x K x 64^2 stays far below 2^31)
   const int bn = regacc ? OZR_BN : OZ_BN;
   static bool attr2 = false;
   if (regacc && !attr2) {
@@ -731,10 +730,6 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
   }
   p.nunits = nu;
   p.group_m = std::max(1, std::min(p.tiles_m, regacc ? 12 : 17));   // sqrt(148 * BN / BM): minimal L2 working set of the tiles in flight
-  {
-    const char* e = getenv("GFCC_OZ_GROUP_M");
-    if (e && atoi(e) > 0) p.group_m = std::min(p.tiles_m, atoi(e));
-  }
   // persistent grid: one CTA per SM of THIS device (the producer rendezvous needs every CTA of the grid to be resident)
   static int dev_sms = 0;
   if (dev_sms == 0) {
@@ -748,8 +743,7 @@ inline cudaError_t oz_igemm(const OzSliced& A, const OzSliced& B, const OzCDesc&
     long long spt = 0;
     for (int u = 0; u < p.nunits; ++u) spt += (long long)p.u[u].np * (p.u[u].kb1 - p.u[u].kb0);
     p.steps_per_tile = (int)spt;
-    static int sync_every = -1;
-    if (sync_every < 0) { const char* e = getenv("GFCC_OZ_SYNC"); sync_every = e ? atoi(e) : 256; }   // 0 switches it off
+    const int sync_every = 256;   // producer rendezvous period in k-blocks (profiles/r1_ozaki.md 2c)
     if (!regacc && sync_every > 0 && sync_buf) {
       cudaError_t e = cudaMemsetAsync(sync_buf, 0, sizeof(unsigned), st);
       if (e != cudaSuccess) return e;

@@ -93,11 +93,16 @@ static int oz_prepare(gfcc_ctx* h, int nrhs) {
     a.base = h->Lov; a.sR = 1; a.sK0 = ov; a.R = (int)ov; a.K0 = Q;               TRY(oz_do_slice(h, a, h->ozLov));
     h->oz_const_ready = true;
   }
-  if (h->oz_ws_nrhs != nrhs || h->oz_ws_ni != h->panel_ni) {
+  if (h->oz_ws_nrhs < nrhs || h->oz_ws_ni != h->panel_ni) {   // capacity semantics, like ensure_workspace()
     oz_release(h, h->ozXU); oz_release(h, h->ozKP);
-    TRY(oz_alloc(h, h->ozXU, (int)ld, (int)ov));
-    TRY(oz_alloc(h, h->ozKP, h->panel_ni * v, (int)ov));
-    h->oz_ws_nrhs = nrhs; h->oz_ws_ni = h->panel_ni;
+    h->oz_ws_nrhs = 0; h->oz_ws_ni = 0;
+    const int cap = std::max(nrhs, h->ws_nrhs);
+    const long long ldcap = (long long)o * 2 * cap;
+    if (ldcap > 2147483647LL) { h->err = "ozaki engine: operand has more than 2^31 rows"; return GFCC_EINVAL; }
+    int rc = oz_alloc(h, h->ozXU, (int)ldcap, (int)ov);
+    if (rc == GFCC_OK) rc = oz_alloc(h, h->ozKP, h->panel_ni * v, (int)ov);
+    if (rc != GFCC_OK) { oz_release(h, h->ozXU); oz_release(h, h->ozKP); return rc; }
+    h->oz_ws_nrhs = cap; h->oz_ws_ni = h->panel_ni;
   }
   return GFCC_OK;
 }
@@ -115,10 +120,11 @@ static int sigma_ring_ozaki(gfcc_ctx* h, int nrhs) {
     CUDA_TRY(h, cudaStreamSynchronize(st));
     if (hf) { h->err = "ozaki engine: tensor-core pipeline wait timed out"; return GFCC_ECUDA; }
   }
-  // XU as B operand: rows (j,c), K = (m,e)
+  // XU as B operand: rows (j,c), K = (m,e); the slice buffer may have room for a wider batch
+  OzSliced xu = oz_rows(h->ozXU, 0, (int)ld);
   {
     OzOperand x; x.base = h->XU; x.sR = 1; x.sK0 = ld; x.R = (int)ld; x.K0 = (int)ov;
-    TRY(oz_do_slice(h, x, h->ozXU));
+    TRY(oz_do_slice(h, x, xu));
   }
   for (int i0 = 0; i0 < o; i0 += h->panel_ni) {
     const int ni = std::min(h->panel_ni, o - i0);
@@ -135,7 +141,7 @@ static int sigma_ring_ozaki(gfcc_ctx* h, int nrhs) {
     // S9: Z[(i,a)][(j,c)] -= K2' XU
     {
       OzCDesc c; c.C = h->Z + (long long)i0 * v * ld; c.sCm0 = ld; c.alpha = -1.0; c.beta = 1.0;
-      TRY(oz_gemm(h, kp, h->ozXU, c));
+      TRY(oz_gemm(h, kp, xu, c));
     }
     // S10: K4[(n,f)][(m,e)] = sum_Q L[Q,m,f] L[Q,n,e];  V[(n,f)][(j,c)] = K4 XU
     {
@@ -145,13 +151,13 @@ static int sigma_ring_ozaki(gfcc_ctx* h, int nrhs) {
     TRY(oz_do_slice(h, kpo, kp));
     {
       OzCDesc c; c.C = h->V + (long long)i0 * v * ld; c.sCm0 = ld;
-      TRY(oz_gemm(h, kp, h->ozXU, c));
+      TRY(oz_gemm(h, kp, xu, c));
     }
   }
   // S11: Z[(i,a)][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]; V takes XU's slice buffer, T2 rows come in batches of panel_ni i's
   {
     OzOperand x; x.base = h->V; x.sR = 1; x.sK0 = ld; x.R = (int)ld; x.K0 = (int)ov;
-    TRY(oz_do_slice(h, x, h->ozXU));
+    TRY(oz_do_slice(h, x, xu));
   }
   for (int i0 = 0; i0 < o; i0 += h->panel_ni) {
     const int ni = std::min(h->panel_ni, o - i0);
@@ -160,7 +166,7 @@ static int sigma_ring_ozaki(gfcc_ctx* h, int nrhs) {
     t.tab = h->blk_tab + (long long)i0 * o; t.sgn = h->blk_sgn + (long long)i0 * o; t.Rb = v; t.tabR = o;
     TRY(oz_do_slice(h, t, tb));
     OzCDesc c; c.C = h->Z + (long long)i0 * v * ld; c.sCm0 = ld; c.beta = 1.0;
-    TRY(oz_gemm(h, tb, h->ozXU, c));
+    TRY(oz_gemm(h, tb, xu, c));
   }
   return GFCC_OK;
 }

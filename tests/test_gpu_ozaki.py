@@ -82,19 +82,32 @@ def test_ozaki_gemm_slices_and_zero_rows():
 @pytest.mark.parametrize("M,N,K", [(300, 520, 20000), (2560, 2560, 17000), (1000, 700, 140000)])
 def test_ozaki_gemm_long_k_kernel(M, N, K):
     """K > 16384 selects the 128 x 256 read-modify-write kernel with the producer rendezvous (more tiles than SMs with a ragged
-    last round, K long enough that one flush unit holds fewer pairs, ragged M/N/K); reference: torch FP64 matmul on the device"""
+    last round, K long enough that one flush unit holds fewer pairs, ragged M/N/K).  Reference: 80-bit long-double dot products
+    on the HOST for a sample of C entries (the four corners, the tile seams at 127/128 and 255/256, random interior entries)."""
     import paper_2010_04768_b200 as g
-    gen = torch.Generator(device="cuda").manual_seed(M + N + K)
-    A = torch.randn((M, K), dtype=torch.float64, device="cuda", generator=gen)
-    B = torch.randn((K, N), dtype=torch.float64, device="cuda", generator=gen)
-    C0 = torch.randn((M, N), dtype=torch.float64, device="cuda", generator=gen)
-    C = C0.clone()
-    g.gfcc_dgemm_ozaki(A, B, C, alpha=-1.0, beta=1.0, nslices=7)
-    ref = C0 - A @ B
-    assert float((C - ref).abs().max() / ref.abs().max()) < 1e-12
-    C = g.gfcc_dgemm_ozaki(A, B, nslices=7)
-    ref = A @ B
-    assert float((C - ref).abs().max() / ref.abs().max()) < 1e-12
+    rng = np.random.default_rng(M + N + K)
+    A = rng.normal(size=(M, K))
+    B = rng.normal(size=(K, N))
+    C0 = rng.normal(size=(M, N))
+    Ad, Bd = dev(A), dev(B)
+    ms = np.concatenate([[0, M - 1, 127 % M, 128 % M], rng.integers(0, M, 60)])
+    ns = np.concatenate([[0, N - 1, 255 % N, 256 % N], rng.integers(0, N, 60)])
+    Al, Bl = A[ms].astype(np.longdouble), B[:, ns].astype(np.longdouble)
+    prod = np.einsum("sk,ks->s", Al, Bl)                                    # exact to 2^-64 per term
+    scale = np.sqrt(K) * 3.0                                                # typical |C| ~ sqrt(K)
+    C = dev(C0)
+    g.gfcc_dgemm_ozaki(Ad, Bd, C, alpha=-1.0, beta=1.0, nslices=7)
+    got = C.cpu().numpy()[ms, ns]
+    ref = (C0[ms, ns].astype(np.longdouble) - prod).astype(np.float64)
+    assert np.abs(got - ref).max() / scale < 1e-12
+    C = g.gfcc_dgemm_ozaki(Ad, Bd, nslices=7)
+    got = C.cpu().numpy()[ms, ns]
+    assert np.abs(got - prod.astype(np.float64)).max() / scale < 1e-12
+    # a NaN / Inf in an operand row must reach the output row (ADVICE r1), not vanish in the slicing
+    A[3, 17] = np.nan
+    B[5, 2] = np.inf
+    C = g.gfcc_dgemm_ozaki(dev(A), dev(B), nslices=7).cpu().numpy()
+    assert np.isnan(C[3]).all() and not np.isfinite(C[:, 2]).any() and np.isfinite(C[4, 3])
 
 
 def _make_pair(s):

@@ -214,6 +214,39 @@ def test_config0_gmres_vs_dense_lu(cfg0):
     assert rr <= 1e-10 and relmax(orc.pack(x1, x2), xs) < 1e-7
 
 
+def test_config0_gmres_residual_history_is_the_krylov_minimum(cfg0):
+    """the residual history returned by the oracle GMRES (used to check the GPU solver step by step) against the DEFINITION
+    of GMRES: after k steps the residual norm is min over the Krylov space span{r0, A r0, ..} of ||r0 - A z||, here from a
+    dense least-squares solve with the assembled 680 x 680 matrix; hist[0] is ||b - A x0|| / ||b||."""
+    s, orc, H = cfg0
+    n = H.shape[0]
+    eta, p, w = s["eta"], s["targets"][1], float(s["omegas"][3])
+    A = H + (w - 1j * eta) * np.eye(n)
+    b = orc.pack(*orc.rhs(p))
+    f = np.diag(np.asarray(s["fock"]))
+    o, v = 8, 24
+    iu = np.triu_indices(o, 1)
+    d = np.concatenate([-f[:o], (f[o:][None, :] - f[iu[0]][:, None] - f[iu[1]][:, None]).reshape(-1)])
+    x0 = b / (w - 1j * eta + d)
+    r0 = b - A @ x0
+    kmax = 12
+    x1, x2, nit, rr, hist = orc.gmres(p, w, eta, 1e-30, m=kmax, maxit=kmax + 1, x0kind=1, history=True)
+    assert nit == kmax + 1 and len(hist) == kmax + 1
+    bn = np.linalg.norm(b)
+    assert abs(hist[0] - np.linalg.norm(r0) / bn) < 1e-12 * hist[0]
+    K = [r0 / np.linalg.norm(r0)]
+    for k in range(1, kmax + 1):
+        Kq, _ = np.linalg.qr(np.stack(K, axis=1))
+        AK = A @ Kq
+        y = np.linalg.lstsq(AK, r0, rcond=None)[0]
+        ref = np.linalg.norm(r0 - AK @ y) / bn
+        assert abs(hist[k] - ref) < 1e-9 * ref, (k, hist[k], ref)
+        nxt = A @ Kq[:, -1]
+        K.append(nxt / np.linalg.norm(nxt))
+    assert (np.diff(hist) <= 1e-15).all()                      # monotone, PAPER.md:136 ("the residual norm decreases monotonically")
+    assert rr == hist[-1]
+
+
 def test_config0_rows_and_physics(cfg0):
     s, orc, H = cfg0
     import gfcc_inputs
