@@ -29,10 +29,27 @@ sys.path.insert(0, ROOT)
 
 import numpy as np  # noqa: E402
 
-FP64_DMMA_PEAK_TFLOPS = 36.95   # measured on this pool's B200: DMMA.8x8x4 issue-rate probe (profiles/fp64_peak_probe.md)
-KFIX = {0: 20, 1: 8, 2: 4, 3: 2, 4: 1}      # Arnoldi steps per timed step (bounded so that a default run ends in minutes)
+FP64_DMMA_PEAK_R1 = 36.95       # round-1 value of the DMMA.8x8x4 issue-rate probe (profiles/fp64_peak_probe.md); the probe is re-run in every bench run
+KFIX = {0: 20, 1: 8, 2: 20, 3: 2, 4: 1}     # Arnoldi steps per timed step (config 2: BASELINE.json "20 GMRES iterations fixed for timing";
+                                            # configs 3-4 bounded so that a default run ends in minutes: one step is 39 s at config 4)
 DEFAULT_CONFIG = 4
-NCU_TRAFFIC_BYTES = {4: 44.098195e9 + 0.131195e9}   # profiles/r1_gemm_ws_ncu_full.md, launch 7
+NCU_TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_gemm_ncu_traffic.csv")   # ncu --set full captures of the step's GEMM launches
+
+
+def ncu_traffic(cfg):
+    """DRAM bytes of the dominant launch shape of a config-`cfg` step, read from the tracked ncu summary (never a constant
+    in this file): the row of NCU_TRAFFIC_CSV with this config whose `dominant` column is 1."""
+    try:
+        import csv
+        with open(NCU_TRAFFIC_CSV) as f:
+            for row in csv.DictReader(l for l in f if not l.startswith("#")):
+                if int(row["config"]) == cfg and int(row["dominant"]) == 1:
+                    return {"bytes": float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), "launch": row["launch"],
+                            "shape": f"{row['M']} x {row['N']} x {row['K']} (BM = {row['BM']})",
+                            "algorithmic_bytes": float(row["algorithmic_bytes"]), "source": os.path.relpath(NCU_TRAFFIC_CSV, ROOT)}
+    except Exception:
+        pass
+    return None
 
 
 def parse():
@@ -45,6 +62,7 @@ def parse():
     ap.add_argument("--kfix", type=int, default=0, help="Arnoldi steps per step (default: per config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-solves", action="store_true", help="skip the converged-solve rate measurement (config 0 and config 1)")
     ap.add_argument("--cpu-baseline-only", action="store_true",
                     help="(internal) child process of the default run: time the oracle sample, print its JSON, exit")
     ap.add_argument("--cpu-baseline-serial", action="store_true",
@@ -104,8 +122,10 @@ def workload_string(cfg, c, nrhs, kfix, rank_shift):
 
 
 # ---------------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, c, nsamp, nrhs_s, ready_cb=None):
-    """time the CPU oracle (as it stands) on a bounded sample of the workload; returns (seconds, description, cores)."""
+def oracle_sample(cfg, c, nrhs_s, ns_small, ns_large, ready_cb=None):
+    """time the CPU oracle (as it stands) on a bounded sample of the workload: the row-sampled sigma at TWO sample sizes
+    (ns_small and ns_large sigma2 rows, each with one sigma1 row and nrhs_s right-hand sides) so that the per-call part
+    (Y, yv over the whole vector) can be separated from the per-row part."""
     import torch
     import gfcc_inputs as gi
     import oracle
@@ -125,24 +145,35 @@ def oracle_sample(cfg, c, nsamp, nrhs_s, ready_cb=None):
     orc = oracle.Oracle(o, v, Q, host["fock"], host["T1"], host["T2p"], host["L1"], host["L2p"], host["Lchol"], oracle.MODE_ROWS)
     t_setup = time.time() - t0
     rng = np.random.default_rng(7)
-    trip = np.stack([rng.integers(0, o - 1, nsamp), np.full(nsamp, o - 1), rng.integers(0, v, nsamp)], axis=1)
-    t0 = time.time()
-    orc.sigma_rows(w, c["eta"], X1, X2, [o - 1], trip)
-    t_rows = time.time() - t0
-    return t_setup, t_rows, trip, oracle.threads()
+    times = []
+    for ns in (ns_small, ns_large):
+        trip = np.stack([rng.integers(0, o - 1, ns), np.full(ns, o - 1), rng.integers(0, v, ns)], axis=1)
+        t0 = time.time()
+        orc.sigma_rows(w, c["eta"], X1, X2, [o - 1], trip)
+        times.append(time.time() - t0)
+    return t_setup, times, oracle.threads()
 
 
 def cpu_baseline(cfg, c, nrhs, flops_sigma, ready_cb=None):
-    nsamp, nrhs_s = (4, 2) if cfg <= 2 else ((2, 1) if cfg == 3 else (1, 1))
-    t_setup, t_rows, trip, cores = oracle_sample(cfg, c, nsamp, nrhs_s, ready_cb)
+    """bounded oracle sample -> extrapolated seconds for ONE batched sigma application of the oracle as it stands:
+    t(ns rows, nrhs_s RHS) = t_call + ns * t_row is fitted to the two timings; a full application is one call with all
+    npair*v rows and nrhs RHS: t_call * (nrhs / nrhs_s) + npair * v * t_row (the row part does not grow with the number of
+    right-hand sides to first order: the row-sampled routine rebuilds O(o^2 v Q) intermediates per row, which is what makes it a
+    checker and not a sigma implementation -- the number is a baseline, not a target)."""
+    nrhs_s = 2
+    ns_small, ns_large = (2, 10) if cfg <= 2 else ((1, 5) if cfg == 3 else (1, 3))
+    t_setup, (t_a, t_b), cores = oracle_sample(cfg, c, nrhs_s, ns_small, ns_large, ready_cb)
+    t_row = max((t_b - t_a) / (ns_large - ns_small), 1e-9)
+    t_call = max(t_a - ns_small * t_row, 0.0)
     npair = c["o"] * (c["o"] - 1) // 2
-    rows_total = npair * c["v"] * nrhs
-    t_full = t_rows * rows_total / (nsamp * nrhs_s)      # linear extrapolation to all rows of all RHS
+    rows_total = npair * c["v"]
+    t_full = t_call * (nrhs / nrhs_s) + rows_total * t_row
     return {"seconds_full": t_full, "value": flops_sigma / t_full / 1e12, "unit": "TFLOP/s", "cores": cores, "kind": "oracle",
-            "sample": (f"row-sampled oracle sigma (oracle/gfcc_oracle.cpp orc_sigma_rows): {nsamp} sigma2 rows + 1 sigma1 row x {nrhs_s} "
-                       f"RHS of config {cfg} in {t_rows:.1f} s (+{t_setup:.1f} s one-time dressing), EXTRAPOLATED linearly to the "
-                       f"{rows_total} (row,RHS) outputs of one batched application"),
-            "seconds_sample": t_rows, "seconds_setup": t_setup}
+            "sample": (f"row-sampled oracle sigma (oracle/gfcc_oracle.cpp orc_sigma_rows) of config {cfg} at two sample sizes: "
+                       f"{ns_small} and {ns_large} sigma2 rows (+1 sigma1 row) x {nrhs_s} RHS in {t_a:.1f} s and {t_b:.1f} s -> per-call part "
+                       f"{t_call:.1f} s, per-row part {t_row:.2f} s (one-time dressing {t_setup:.1f} s, not charged); one batched application = "
+                       f"{rows_total} rows x {nrhs} RHS in one call: EXTRAPOLATED by a factor {rows_total / ns_large:.3g} in the row count"),
+            "seconds_per_row": t_row, "seconds_per_call": t_call, "seconds_setup": t_setup, "extrapolation_factor": rows_total / ns_large}
 
 
 def model_flops(c, nrhs):
@@ -168,13 +199,10 @@ def run_cpu_baseline_child(args):
 
 
 def start_cpu_baseline_child(cfg):
-    """start the oracle timing BESIDE the GPU part (the GPU part is timed on the device with CUDA events and its launches
-    are 10-300 ms long, so host contention does not reach it); the oracle gets all host cores but two."""
-    cores = os.cpu_count() or 4
-    env = dict(os.environ)
-    env["OMP_NUM_THREADS"] = str(max(1, cores - 2))
+    """start the oracle timing in a child process on ALL host cores.  It overlaps only the untimed GPU phases of this run (input
+    generation, gfcc_create, warm-up): main() waits for it BEFORE the timed region starts, so neither measurement disturbs the other."""
     child = subprocess.Popen([sys.executable, os.path.abspath(__file__), "--cpu-baseline-only", "--config", str(cfg)],
-                             stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, env=env)
+                             stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, env=dict(os.environ))
     while True:                                   # wait until the child has released the device memory of its inputs
         ln = child.stdout.readline()
         if not ln or ln.strip() == "READY":
@@ -182,7 +210,7 @@ def start_cpu_baseline_child(cfg):
     return child
 
 
-def finish_cpu_baseline_child(child, flops_sigma, timeout_s=900):
+def finish_cpu_baseline_child(child, flops_sigma, timeout_s=1800):
     try:
         out, _ = child.communicate(timeout=timeout_s)
     except subprocess.TimeoutExpired:
@@ -192,9 +220,7 @@ def finish_cpu_baseline_child(child, flops_sigma, timeout_s=900):
         if ln.startswith("{"):
             cb = json.loads(ln)
             cb["value"] = flops_sigma / cb.pop("seconds_full") / 1e12
-            cb["sample"] += "; timed in a child process BESIDE the GPU part of this run (OMP threads = host cores - 2)"
-            cb.pop("seconds_sample", None)
-            cb.pop("seconds_setup", None)
+            cb["sample"] += "; timed in a child process on all host cores during input generation / gfcc_create / warm-up, finished before the timed region"
             return cb
     return {"value": None, "unit": "TFLOP/s", "cores": None, "kind": "oracle", "sample": "oracle child printed no result"}
 
@@ -220,7 +246,7 @@ def run_reference(args):
         if it >= args.warmup:
             vals.append(cb["value"])
         last = cb
-        if it == 0 and cb["seconds_sample"] + cb["seconds_setup"] > 60:
+        if it == 0 and cb["seconds_setup"] + cb["seconds_per_call"] + 4 * cb["seconds_per_row"] > 60:
             # one sample already takes a minute: do not repeat it warmup+steps times
             vals = [cb["value"]]
             break
@@ -232,9 +258,50 @@ def run_reference(args):
             "config": {"workload": workload_string(cfg, c, nrhs, kfix, 0), "l2": "working set >> 126 MB L2"},
             "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
             "e2e": {"value": value, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0, "note": f"extrapolated from sampled rows ({npair_rows} outputs per application)"}
+            "gpu_launches": 0, "note": f"extrapolated from sampled rows ({npair_rows} outputs per application; factor {last['extrapolation_factor']:.3g})"}
     print(json.dumps(line))
     return 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+def converged_solves(g, gi, torch, stream):
+    """(p,omega) solves per second from CONVERGED batched GMRES solves (gfcc_solve_ip to the config's own tolerance, compaction and
+    refill on): config 0 inside its own omega window (4 p x 8 omega, tol 1e-10) and config 1 at omega above the poles, where the
+    paper's unpreconditioned GMRES converges on the synthetic spectrum (reading 23; 16 p x 2 omega, tol 1e-8)."""
+    out = {}
+    for name, cfg, ws, m in (("config0", 0, None, 400), ("config1", 1, [0.4, 0.5], 700)):
+        c = gi.CONFIGS[cfg]
+        s = gi.make_config(cfg, "cuda")
+        h = g.gfcc_create(c["o"], c["v"], c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+        g.gfcc_set_stream(h, stream)
+        g.gfcc_set_option(h, "gmres_m", m)
+        g.gfcc_set_option(h, "gmres_maxit", 4 * m)
+        omegas = np.linspace(c["wlo"], c["whi"], c["nw"]) if ws is None else np.array(ws)
+        targets = gi.targets(cfg)
+        res = {}
+        for label, comp in (("lockstep", -1.0), ("compaction", 0.125)):
+            g.gfcc_set_option(h, "compact", comp)
+            g.gfcc_solve_ip(h, targets, omegas, c["eta"], c["tol"], allow_noconv=True)          # warm-up (allocations)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                e0.record(stream)
+                g.gfcc_solve_ip(h, targets, omegas, c["eta"], c["tol"], allow_noconv=True)
+                e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            n = len(targets) * len(omegas)
+            rel, its = g.gfcc_get_residuals(h, n)
+            res[label] = {"ms": ms, "solves_per_s": n / (ms * 1e-3), "n_unconverged": int(g.gfcc_get_stat(h, "n_unconverged")),
+                          "iterations_min_max": [int(its.min()), int(its.max())], "compactions": int(g.gfcc_get_stat(h, "compactions")),
+                          "col_steps": g.gfcc_get_stat(h, "active_col_steps"), "lockstep_col_steps": g.gfcc_get_stat(h, "lockstep_col_steps")}
+        best = max(res.values(), key=lambda r: r["solves_per_s"])
+        out[name] = {"solves": len(targets) * len(omegas), "omega": [float(omegas[0]), float(omegas[-1])], "tol": c["tol"], "gmres_m": m,
+                     "solves_per_s": best["solves_per_s"], **res}
+        g.gfcc_destroy(h)
+        del s
+        torch.cuda.empty_cache()
+    return out
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -267,7 +334,7 @@ def main():
     nrhs = c["np"] * c["nw"]
     kfix = args.kfix or KFIX[cfg]
 
-    # ---- CPU baseline: started first, runs beside the GPU part (rank 0, N = 1 only) ----
+    # ---- CPU baseline: started first; overlaps only input generation / gfcc_create / warm-up (rank 0, N = 1 only) ----
     cpu_child = None
     if world == 1 and not args.no_cpu_baseline and not args.cpu_baseline_serial:
         cpu_child = start_cpu_baseline_child(cfg)
@@ -313,6 +380,12 @@ def main():
     for _ in range(args.warmup):
         step()
     flops_sigma = g.gfcc_get_stat(h, "flops_sigma")
+    # roofline denominator measured IN THIS RUN: DMMA issue-rate probe on the same GPU, same stream, just before the timed region
+    peak_in_run = g.gfcc_probe_fp64_peak(20000, 3, stream)
+    cpu_result = None
+    if cpu_child is not None:                       # the oracle sample must be over before the timed region starts
+        cpu_result = finish_cpu_baseline_child(cpu_child, flops_sigma)
+        cpu_child = None
     g.gfcc_get_stat(h, "reset_counters")
     overlap_on = args.overlap == 1
     if not overlap_on:      # per-launch events serialise the side streams, so with overlap the GEMM profile is a separate step
@@ -350,7 +423,7 @@ def main():
     ms_step = ms_total / args.steps
     apps_per_step = napply / args.steps
     value = world * apps_per_step * flops_sigma / (ms_step * 1e-3) / 1e12
-    solves_per_s = world * nrhs / (ms_step * 1e-3)
+    rhs_steps_per_s = world * nrhs * kfix / (ms_step * 1e-3)
 
     line = {
         "metric": "sigma_matvec_fp64_tflops", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
@@ -359,13 +432,18 @@ def main():
         "config": {"workload": workload_string(cfg, c, nrhs, kfix, rank), "l2": "inputs and working set >> 126 MB L2 (no flush needed)",
                    "flop_model": "executed Cholesky-route model, SURVEY.md 8(d): real x complex = 2 real products, pair-packed o^4 term",
                    "flops_per_sigma_application": flops_sigma, "sigma_applications_per_step": apps_per_step,
-                   "gmres_m_used": g.gfcc_get_stat(h, "gmres_m_used"), "overlap": int(overlap_on),
-                   "gemm_engine": (os.environ.get("GFCC_GEMM_ENGINE", "ws") if args.engine == "dmma" else
+                   "gmres_fixed_steps": kfix, "gmres_m_memory_limit": g.gfcc_get_stat(h, "gmres_m_memory_limit"),
+                   "gmres_m_note": "gmres_m_memory_limit = longest Krylov basis (batch vectors) the free device memory allows beside the "
+                                   "resident intermediates at this batch width; the timed step runs gmres_fixed_steps Arnoldi steps",
+                   "overlap": int(overlap_on),
+                   "gemm_engine": ("dgemm_ws_kernel (FP64 DMMA, warp-specialised)" if args.engine == "dmma" else
                                    f"ozaki_int8 x{args.slices} slices for S6, S8-S11 (tcgen05.mma kind::i8, exact int32 accumulation, FP64-accurate; "
                                    "NOT the graded FP64 DMMA engine), rest on the DMMA engine"),
                    "panel_ni": g.gfcc_get_stat(h, "panel_ni")},
-        "solves_per_s": solves_per_s, "solves_note": f"(p,omega) right-hand sides advanced by {kfix} GMRES steps per second x nrhs",
-        "pct_fp64_peak_measured": 100.0 * value / world / FP64_DMMA_PEAK_TFLOPS,
+        "rhs_arnoldi_steps_per_s": rhs_steps_per_s,
+        "rhs_arnoldi_steps_note": "(right-hand sides x Arnoldi steps) per second in the fixed-step timing mode; NOT a solve rate -- "
+                                  "converged (p,omega) solves per second are in `solves`",
+        "pct_fp64_peak_measured": 100.0 * value / world / peak_in_run,
         "create_s": create_s, "create_tflops": flops_create / create_s / 1e12, "inputs_s": t_inputs,
         "device_bytes": g.gfcc_get_stat(h, "bytes_device"), "gpu_launches": int(launches),
     }
@@ -376,19 +454,22 @@ def main():
     achieved = gemm_flops / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
     line["roofline"] = {
         "kernel": "gfcc::dgemm_ws_kernel (all GEMM-engine launches of the timed region)",
-        "bound": "tensor", "achieved": achieved, "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_DMMA_PEAK_TFLOPS,
-        "peak_source": "measured FP64 DMMA.8x8x4 issue-rate ceiling on this pool's B200 (profiles/fp64_peak_probe.md); "
-                       "MEASURED_PEAKS.json has no FP64 entry",
+        "bound": "tensor", "achieved": achieved, "peak": peak_in_run, "unit": "TFLOP/s", "frac": achieved / peak_in_run,
+        "peak_source": "FP64 DMMA.8x8x4 issue-rate ceiling measured IN THIS RUN by gfcc_probe_fp64_peak (register-only DMMA loop on every SM, "
+                       "CUDA events, right before the timed region); MEASURED_PEAKS.json has no FP64 entry",
+        "peak_round1_constant": FP64_DMMA_PEAK_R1,
         "peak_alt_bf16_ratio": (mp["bf16_tflops_sustained"] * 40.0 / 2250.0) if mp else None,
         "peak_alt_note": "sustained bf16 peak of MEASURED_PEAKS.json x nominal FP64:bf16 ratio 40/2250 (fallback rule; lower than the "
                          "directly measured DMMA ceiling, so the stricter denominator is used for frac)",
         "launches": int(gemm_n), "avg_launch_ms": gemm_ms / max(gemm_n, 1), "share_of_step": gemm_ms / ms_prof if ms_prof > 0 else None,
-        "algorithmic_flops": gemm_flops, "traffic": NCU_TRAFFIC_BYTES.get(cfg),
-        "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel from ncu --set full "
-                        "(profiles/r1_gemm_ws_ncu_full.md): the config-4 S9 panel GEMM 2640 x 5760 x 118800 (the most frequent big launch of a "
-                        "step), whose algorithmic bytes (A + B + C once) are 8.2e9; DRAM is 4.9 % busy in that launch (tensor-bound, 91.7 % DMMA "
-                        "pipe), L2 hit 80 %; null for configs without a capture",
+        "algorithmic_flops": gemm_flops,
     }
+    tr = ncu_traffic(cfg)
+    line["roofline"]["traffic"] = tr["bytes"] if tr else None
+    line["roofline"]["traffic_note"] = (
+        f"dram__bytes_read.sum + dram__bytes_write.sum of ONE launch from ncu --set full, read from {tr['source']}: launch '{tr['launch']}', "
+        f"{tr['shape']}, the most frequent big launch of this step; its algorithmic bytes (A + B + C once) are {tr['algorithmic_bytes']:.3g}"
+        if tr else "no ncu capture of this config's launch shapes in profiles/r2_gemm_ncu_traffic.csv")
 
     if args.engine == "ozaki" and oz_ms > 0:
         i8_peak = (mp["bf16_tflops_sustained"] * 2.0) if mp else 2.0 * 1365.7
@@ -417,7 +498,7 @@ def main():
             S1p = torch.empty(X1h.shape, dtype=X1h.dtype, pin_memory=True)
             S2p = torch.empty(X2h.shape, dtype=X2h.dtype, pin_memory=True)
             g.gfcc_sigma_ip_host(h, wr, c["eta"], X1h.numpy(), X2h.numpy(), out=(S1p, S2p))   # warm-up
-            nrep = 1 if cfg >= 3 else 3
+            nrep = 2 if cfg >= 3 else 3
             t0 = time.perf_counter()
             for _ in range(nrep):
                 S1h, S2h = g.gfcc_sigma_ip_host(h, wr, c["eta"], X1h.numpy(), X2h.numpy(), out=(S1p, S2p))
@@ -460,14 +541,21 @@ def main():
     del s
     torch.cuda.empty_cache()
 
+    # ---- converged (p,omega) solves per second: real batched solves to the config's tolerance (rank 0, N = 1) ----
+    if world == 1 and not args.no_solves:
+        try:
+            line["solves"] = converged_solves(g, gi, torch, stream)
+            line["solves_per_s"] = line["solves"]["config0"]["solves_per_s"]
+        except Exception as ex:   # noqa: BLE001
+            line["solves"] = {"error": str(ex)[:200]}
+
     # ---- CPU baseline: the oracle on the host cores, bounded sample (rank 0, N = 1 only) ----
-    if cpu_child is not None:
-        line["cpu_baseline"] = finish_cpu_baseline_child(cpu_child, flops_sigma)
+    if cpu_result is not None:
+        line["cpu_baseline"] = cpu_result
     elif world == 1 and not args.no_cpu_baseline:
         try:
             cb = cpu_baseline(cfg, c, nrhs, flops_sigma)
-            for k in ("seconds_sample", "seconds_setup", "seconds_full"):
-                cb.pop(k, None)
+            cb.pop("seconds_full", None)
             line["cpu_baseline"] = cb
         except Exception as ex:   # noqa: BLE001
             line["cpu_baseline"] = {"value": None, "unit": "TFLOP/s", "cores": None, "kind": "oracle", "sample": f"failed: {str(ex)[:200]}"}

@@ -1,10 +1,14 @@
-"""Micro-benchmarks of the building blocks (B200): FP64 DMMA ceiling, the GEMM engine on square and on the sigma-shaped
+"""Measurement tool (not product): micro-benchmarks of the building blocks (B200): FP64 DMMA ceiling, the GEMM engine on square and on the sigma-shaped
 problems of a config, HBM copy.  Used for the roofline notes in DESIGN.md / profiles/ and as the short command ncu wraps.
 
-    python -m paper_2010_04768_b200.microbench [--probe] [--square N] [--sigma-shapes CFG] [--ozaki-shapes CFG] [--slices S] [--reps R]
+    python bench_micro.py [--probe] [--square N] [--sigma-shapes CFG] [--ozaki-shapes CFG] [--slices S] [--reps R]
 """
 import argparse
 import json
+import os
+import sys
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 import torch
 

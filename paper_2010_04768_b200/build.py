@@ -12,7 +12,7 @@ LIB = os.path.join(HERE, "libgfcc_b200.so")
 SOURCES = ["gfcc_lib.cu"]
 DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".inl", ".h"))) + [os.path.join("..", "..", "include", "gfcc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-ldl"]
 
 
 def _newest_dep():

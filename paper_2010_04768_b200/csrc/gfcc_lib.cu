@@ -10,6 +10,7 @@
 // on the fly from the Cholesky vectors (never stored; BASELINE.json configs[2..4]).  No CPU fallback.
 // =====================================================================================
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -27,6 +28,14 @@
 #include "gfcc_ozaki.cuh"
 
 using namespace gfcc;
+
+// NVTX range per sigma term / create phase / solver phase (the paper times get / compute / add per
+// iteration, Table 4; here the phases are the rows of SURVEY.md 8a).  Header-only NVTX v3: a no-op unless a
+// profiler is attached.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 static thread_local std::string g_create_error;
 
@@ -274,12 +283,14 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   double* KPb = par ? h->KP2 : h->KP;
   struct Restore { gfcc_ctx* h; ~Restore() { h->cur = h->stream; } } restore{h};
 
+  NvtxRange nv_sigma("gfcc sigma (S1-S13)");
   h->cur = s0;
   // XU[m][e][j][c] = x2[m,j,e]
   k_unpack_xu<<<(unsigned)ov, 256, 0, s0>>>(h->XU, xin, o, v, (int)Nc);
   KLAUNCH(h);
   // S1: Y[Q][(j,c)] = sum_(m,e) Lov[Q][(m,e)] XU[(m,e)][(j,c)]
   {
+    NvtxRange nv("S1 Y = Lov XU");
     GemmDesc d; d.M = Q; d.N = (int)ld; d.K0 = (int)ov;
     d.A = h->Lov; d.sAm = ov; d.sAk0 = 1;
     d.B = h->XU; d.sBk0 = ld; d.sBn = 1;
@@ -293,6 +304,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   }
   // S7: Z[(i,a)][(j,c)] = sum_Q Lm[Q][(i,a)] Y[Q][(j,c)]
   {
+    NvtxRange nv("S7 Z13 = Lm^T Y");
     GemmDesc d; d.M = (int)ov; d.N = (int)ld; d.K0 = Q;
     d.A = h->Lm; d.sAm = 1; d.sAk0 = ov;
     d.B = h->Y; d.sBk0 = ld; d.sBn = 1;
@@ -302,6 +314,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   if (oz) TRY(sigma_ring_ozaki(h, nrhs));
   for (int i0 = 0; i0 < o && !oz; i0 += h->panel_ni) {
     const int ni = std::min(h->panel_ni, o - i0);
+    NvtxRange nv_panel("S8-S10 panel (K2 build, Z -= K2 XU, K4 build, V = K4 XU)");
     // ---- chain A: S8+S9 (+S3,S4 folded): panel of K2'[(i,a)][(m,e)], Z -= K2' XU
     h->cur = s0;
     {
@@ -342,6 +355,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   h->cur = sC;
   // S12a: yv[e][c] = - sum_(Q,m) Lov[Q][m][e] Y[Q][m][c]
   {
+    NvtxRange nv("S12a yv");
     GemmDesc d; d.M = v; d.N = (int)Nc; d.K1 = Q; d.K0 = o;
     d.A = h->Lov; d.sAm = 1; d.sAk0 = v; d.sAk1 = ov;
     d.B = h->Y; d.sBk0 = Nc; d.sBk1 = ld; d.sBn = 1;
@@ -349,6 +363,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     TRY(gemm_splitk(h, d, 64));
   }
   // S2: sigma1[i][c] = sum_(Q,n) Loo[Q,n,i] Y[Q][n][c]  -  sum_(m,e) Fme[m,e] XU[(m,e)][(i,c)]  + small terms
+  nvtxRangePushA("S2 sigma1");
   {
     GemmDesc d; d.M = o; d.N = (int)Nc; d.K1 = Q; d.K0 = o;
     d.A = h->LooT; d.sAm = o; d.sAk0 = 1; d.sAk1 = (long long)o * o;
@@ -365,11 +380,13 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     TRY(gemm_splitk(h, d, 32));
   }
   k_sigma1_small<<<(unsigned)((o * nrhs + 127) / 128), 128, 0, sC>>>(sout, xin, h->Fmi, d_omega, eta, o, nrhs);
+  nvtxRangePop();
   KLAUNCH(h);
   // S6 (D): s2[(i<j)][(a,c)] = sum_(m<n) W[(i<j)][(m<n)] x2[(m<n)][(a,c)]
   bool s6_done = false;
   if (oz) TRY(sigma_s6_ozaki(h, nrhs, x2, s2, &s6_done));
   if (!s6_done) {
+    NvtxRange nv("S6 W_mnij x2");
     GemmDesc d; d.M = (int)h->npair; d.N = (int)(v * Nc); d.K0 = (int)h->npair;
     d.A = h->Wp; d.sAm = h->npair; d.sAk0 = 1;
     d.B = x2; d.sBk0 = v * Nc; d.sBn = 1;
@@ -378,6 +395,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   }
   // S12b (F): s2[(pair,a)][c] += sum_e t[(pair),a,e] yv[e][c]
   {
+    NvtxRange nv("S12b T2 yv");
     GemmDesc d; d.M = (int)(h->npair * v); d.N = (int)Nc; d.K0 = v;
     d.A = h->T2p; d.sAm = v; d.sAk0 = 1;
     d.B = h->yv; d.sBk0 = Nc; d.sBn = 1;
@@ -386,6 +404,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   }
   // S5 (C): s2[(pair,a)][c] += sum_m WB[(pair,a)][m] x1[m][c]
   {
+    NvtxRange nv("S5 W_mbij x1");
     GemmDesc d; d.M = (int)(h->npair * v); d.N = (int)Nc; d.K0 = o;
     d.A = h->WB; d.sAm = o; d.sAk0 = 1;
     d.B = xin; d.sBk0 = Nc; d.sBn = 1;
@@ -402,6 +421,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   }
   // S11: Z[i][a][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]   (T2 blocks through the pair table, sign per block)
   if (!oz) {
+    NvtxRange nv("S11 Z4 = T2 V");
     GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
     d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
     d.tabs_even = ((long long)v * v) % 2 == 0;
@@ -411,6 +431,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
     TRY(gemm(h, d));
   }
   // S13: shift + P(ij) ring
+  NvtxRange nv_s13("S13 epilogue");
   k_sigma2_epilogue<<<(unsigned)h->npair, 256, 0, s0>>>(sout, xin, h->Z, d_omega, eta, o, v, nrhs);
   KLAUNCH(h);
   h->st_sigma_apps += 1;
@@ -478,6 +499,7 @@ static int create_impl(gfcc_ctx* h, const double* fock, const double* T1, const 
     k_copy_block<<<grid, blk, 0, st>>>(dst, Lchol, R, Cc, row0, col0, N, transpose);
   };
   // ---- P1: T1-dressed Cholesky blocks ----
+  nvtxRangePushA("gfcc_create P1-P2 (dressing)");
   copy_block(h->Lov, o, v, 0, o, 0); KLAUNCH(h);          // Lov[Q][m][e] = L[Q][m][o+e]
   copy_block(h->LooT, o, o, 0, 0, 1); KLAUNCH(h);         // LooT[Q][i][m] = L[Q][m][i]
   copy_block(h->Lvv, v, v, o, o, 0); KLAUNCH(h);          // Lvv[Q][a][e] = L[Q][o+a][o+e]
@@ -541,6 +563,8 @@ static int create_impl(gfcc_ctx* h, const double* fock, const double* T1, const 
   dev_free(h, sq, Q); dev_free(h, U, (long long)Q * N * o); dev_free(h, Kmat, (long long)N * N);
   dev_free(h, g, (long long)N * N); dev_free(h, tmp, (long long)N * N); dev_free(h, ft, (long long)N * N);
 
+  nvtxRangePop();
+  NvtxRange nv_p37("gfcc_create P3-P7");
   // ---- P3: Mq[Q][i][a] = sum_(n,f) t[i,n,f,a] Lov[Q][n][f]   (batch over i, T2 blocks via the pair table on B)
   double* Mq = nullptr;
   TRY(dev_alloc(h, &Mq, Q * ov));
