@@ -46,6 +46,14 @@ def lib():
                                 ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_double_p, _c_double_p, _c_double_p]
         L.orc_gmres_hist.restype = ctypes.c_int
         L.orc_gmres_hist.argtypes = L.orc_gmres.argtypes + [_c_double_p, ctypes.c_int]
+        L.orc_sigma_ea.argtypes = [ctypes.c_void_p, ctypes.c_int, _c_double_p, ctypes.c_double] + [_c_double_p] * 4
+        L.orc_rhs_ea.argtypes = [ctypes.c_void_p, ctypes.c_int, _c_double_p, _c_double_p]
+        L.orc_bra_ea.argtypes = [ctypes.c_void_p, ctypes.c_int, _c_double_p, _c_double_p]
+        L.orc_bra_dot_ea.argtypes = [ctypes.c_void_p] + [_c_double_p] * 5
+        L.orc_gmres_ea.restype = ctypes.c_int
+        L.orc_gmres_ea.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                   ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_double_p, _c_double_p, _c_double_p,
+                                   _c_double_p, ctypes.c_int]
         L.orc_sigma_rows.argtypes = [ctypes.c_void_p, ctypes.c_int, _c_double_p, ctypes.c_double, _c_double_p,
                                      _c_double_p, ctypes.c_int, _c_int_p, _c_double_p, ctypes.c_int, _c_int_p,
                                      _c_double_p]
@@ -59,6 +67,7 @@ def threads() -> int:
 
 MODE_DEF = 1      # definition form (items 1-7 with explicit <pq||rs> blocks)
 MODE_ROWS = 2     # T1-dressed factorised form for row-sampled sigma
+MODE_EA = 4       # with MODE_DEF: EA / advanced-part intermediates (W_amef, W_abef, W_abei; O(v^4) memory)
 
 
 class Oracle:
@@ -92,7 +101,8 @@ class Oracle:
         lib().orc_get(self.h, name.encode(), _dp(out))
         o, v, N = self.o, self.v, self.N
         shapes = dict(Fme=(o, v), Fmi=(o, o), Fae=(v, v), Wmnij=(o, o, o, o), Wmnie=(o, o, o, v),
-                      Wmbej=(o, v, v, o), Wmbij=(o, v, o, o), oovv=(o, o, v, v), ft=(N, N))
+                      Wmbej=(o, v, v, o), Wmbij=(o, v, o, o), oovv=(o, o, v, v), ft=(N, N),
+                      Wamef=(v, o, v, v), Wabef=(v, v, v, v), Wabei=(v, v, v, o))
         return out.reshape(shapes[name])
 
     # ---- sigma ---------------------------------------------------------------------------
@@ -211,4 +221,98 @@ class Oracle:
         for iw, w in enumerate(omegas):
             X = np.linalg.solve(H + (w - 1j * eta) * np.eye(n), B)
             G[iw] = (C.T @ X).T          # [ip, iq]
+        return G
+
+    # ---- EA / advanced part (Eq. 6; second terms of Eq. 7-8) ---------------------------------
+    # vectors: y1 [v], y2 [o, v, v] (index order j, a, b; antisymmetric in a, b); packed basis: 1p then (j, a<b), j slowest
+    def sigma_ea(self, omega, eta, Y1, Y2):
+        """sigma_EA = (omega + i eta) Y - Hbar Y.  Y1 [nrhs,v], Y2 [nrhs,o,v,v] complex128 -> (S1, S2)."""
+        Y1 = np.ascontiguousarray(Y1, dtype=np.complex128)
+        Y2 = np.ascontiguousarray(Y2, dtype=np.complex128)
+        nrhs = Y1.shape[0]
+        om = np.ascontiguousarray(np.broadcast_to(np.asarray(omega, dtype=np.float64), (nrhs,)))
+        S1 = np.empty_like(Y1)
+        S2 = np.empty_like(Y2)
+        rc = lib().orc_sigma_ea(self.h, nrhs, _dp(om), float(eta), _dp(Y1.view(np.float64)), _dp(Y2.view(np.float64)),
+                                _dp(S1.view(np.float64)), _dp(S2.view(np.float64)))
+        if rc:
+            raise RuntimeError("orc_sigma_ea needs MODE_DEF | MODE_EA")
+        return S1, S2
+
+    def rhs_ea(self, q):
+        b1 = np.empty(self.v, dtype=np.complex128)
+        b2 = np.empty((self.o, self.v, self.v), dtype=np.complex128)
+        if lib().orc_rhs_ea(self.h, int(q), _dp(b1.view(np.float64)), _dp(b2.view(np.float64))):
+            raise ValueError("q out of range")
+        return b1, b2
+
+    def bra_ea(self, p):
+        c1 = np.empty(self.v)
+        c2 = np.empty((self.o, self.v, self.v))
+        if lib().orc_bra_ea(self.h, int(p), _dp(c1), _dp(c2)):
+            raise ValueError("p out of range")
+        return c1, c2
+
+    def bra_dot_ea(self, c1, c2, y1, y2):
+        out = np.empty(1, dtype=np.complex128)
+        y1 = np.ascontiguousarray(y1, dtype=np.complex128)
+        y2 = np.ascontiguousarray(y2, dtype=np.complex128)
+        lib().orc_bra_dot_ea(self.h, _dp(c1), _dp(c2), _dp(y1.view(np.float64)), _dp(y2.view(np.float64)),
+                             _dp(out.view(np.float64)))
+        return out[0]
+
+    def pack_ea(self, y1, y2):
+        au = np.triu_indices(self.v, 1)
+        return np.concatenate([np.asarray(y1).reshape(-1), np.asarray(y2)[:, au[0], au[1]].reshape(-1)])
+
+    def unpack_ea(self, z):
+        o, v = self.o, self.v
+        y1 = z[:v].copy()
+        y2 = np.zeros((o, v, v), dtype=z.dtype)
+        au = np.triu_indices(v, 1)
+        blk = z[v:].reshape(o, -1)
+        y2[:, au[0], au[1]] = blk
+        y2[:, au[1], au[0]] = -blk
+        return y1, y2
+
+    def gmres_ea(self, q, omega, eta, tol, m=50, maxit=1000, x0kind=1, history=False):
+        y1 = np.empty(self.v, dtype=np.complex128)
+        y2 = np.empty((self.o, self.v, self.v), dtype=np.complex128)
+        rr = np.empty(1)
+        hist = np.full(int(maxit) + 1, np.nan)
+        n = lib().orc_gmres_ea(self.h, int(q), float(omega), float(eta), float(tol), int(m), int(maxit), int(x0kind),
+                               _dp(y1.view(np.float64)), _dp(y2.view(np.float64)), _dp(rr), _dp(hist), len(hist))
+        if n < 0:
+            raise RuntimeError("orc_gmres_ea needs MODE_DEF | MODE_EA")
+        return (y1, y2, n, rr[0], hist[:n]) if history else (y1, y2, n, rr[0])
+
+    def dense_hbar_ea(self):
+        """Real matrix of Hbar_EA in the packed basis: column nu = -(sigma_EA(e_nu) at omega = eta = 0)."""
+        n = self.v + self.o * self.ntri
+        H = np.empty((n, n))
+        bs = 64
+        for c0 in range(0, n, bs):
+            c1 = min(n, c0 + bs)
+            Y1 = np.zeros((c1 - c0, self.v), dtype=np.complex128)
+            Y2 = np.zeros((c1 - c0, self.o, self.v, self.v), dtype=np.complex128)
+            for k in range(c0, c1):
+                e = np.zeros(n, dtype=np.complex128)
+                e[k] = 1.0
+                Y1[k - c0], Y2[k - c0] = self.unpack_ea(e)
+            S1, S2 = self.sigma_ea(0.0, 0.0, Y1, Y2)
+            for k in range(c0, c1):
+                H[:, k] = -self.pack_ea(S1[k - c0], S2[k - c0]).real
+        return H
+
+    def G_dense_ea(self, plist, omegas, eta, H=None):
+        """advanced part G^A[w, ip, iq] = c_p^T ((omega + i eta) 1 - Hbar_EA)^-1 b_q by dense LU (second term of Eq. 2 / 8)."""
+        if H is None:
+            H = self.dense_hbar_ea()
+        n = H.shape[0]
+        B = np.stack([self.pack_ea(*self.rhs_ea(q)) for q in plist], axis=1)
+        C = np.stack([self.pack_ea(*self.bra_ea(p)) for p in plist], axis=1)
+        G = np.empty((len(omegas), len(plist), len(plist)), dtype=np.complex128)
+        for iw, w in enumerate(omegas):
+            Y = np.linalg.solve((w + 1j * eta) * np.eye(n) - H, B)      # columns q
+            G[iw] = C.T @ Y                                              # [ip, iq]
         return G

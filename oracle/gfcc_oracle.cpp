@@ -54,6 +54,10 @@ struct Ctx {
   std::vector<double> Lt;                                         // [p][r][Q]
   std::vector<double> oooo, ooov, oovv, ovvo, ovvv, ovoo;         // <pq||rs> blocks
   std::vector<double> Fme, Fmi, Fae, Wmnij, Wmnie, Wmbej, Wmbij;  // items 1-7
+  // ---- EA / advanced part, definition form (mode bit 2) ----
+  bool has_ea = false;
+  std::vector<double> vvvv, vvvo;                 // <ab||ef>, <ab||ei>
+  std::vector<double> Wamef, Wabef, Wabei;        // EA intermediates (build_ea)
   // ---- sampled (factorised, T1-dressed) form ----
   bool has_dressed = false;
   std::vector<double> Loo, Lov, Lvv, Lvo;  // dressed blocks, layout [m][i][Q], [m][e][Q], [a][e][Q], [a][i][Q]
@@ -416,12 +420,223 @@ inline double dotQ(const double* a, const double* b, int Q) {
   return acc;
 }
 
+// ------------------------------------------------------------------------------------
+// EA / advanced part (Eq. 4, Eq. 6, second terms of Eq. 7-8), definition form.
+// Operator Y = sum_a y1[a] a+_a + sum_{j, a<b} y2[j,a,b] a+_a a+_b a_j  (Eq. 4 order; y2 antisymmetric in a,b).
+// The paper prints no working equations (reading 28); these are the spin-orbital EA-EOM-CCSD-type
+// equations for the connected action <mu|[Hbar_N, Y]|Phi>, pinned by the Fock-space brute force in tests/:
+//   W_amef = <am||ef> - sum_n t[n,a] <nm||ef>
+//   W_abef = <ab||ef> - P(ab) sum_m t[m,b] <am||ef> + 1/2 sum_mn tau[m,n,a,b] <mn||ef>
+//   W_abei = <ab||ei> + 1/2 sum_mn <mn||ei> tau[m,n,a,b] - sum_m F_me t[m,i,a,b] + sum_f W_abef t[i,f]
+//            - P(ab) sum_mf <mb||ef> t[m,i,a,f] - P(ab) sum_m t[m,a] ( <mb||ei> - sum_nf t[n,i,b,f] <mn||ef> )
+//   (Hbar y)1[a]     = sum_c F_ac y1[c] + sum_ld F_ld y2[l,a,d] + 1/2 sum_lcd W_alcd y2[l,c,d]
+//   (Hbar y)2[j,a,b] = sum_c W_abcj y1[c] + P(ab) sum_c F_ac y2[j,c,b] - sum_l F_lj y2[l,a,b] + P(ab) sum_ld W_lbdj y2[l,a,d]
+//                      + 1/2 sum_cd W_abcd y2[j,c,d] - 1/2 sum_klcd <kl||cd> y2[l,c,d] t[k,j,a,b]
+//   sigma_EA = (omega + i eta) y - Hbar y                                                      (Eq. 6)
+// ------------------------------------------------------------------------------------
+void build_ea(Ctx& c) {
+  const int o = c.o, v = c.v;
+  build_block(c, c.vvvv, o, v, o, v, o, v, o, v);
+  build_block(c, c.vvvo, o, v, o, v, o, v, 0, o);
+  const std::vector<double>&t1 = c.t1, &t2 = c.t2;
+  auto T1 = [&](int i, int a) { return t1[(i64)i * v + a]; };
+  auto T2 = [&](int i, int j, int a, int b) { return t2[IDX4(i, j, a, b, o, v, v)]; };
+  auto TAU = [&](int i, int j, int a, int b) { return T2(i, j, a, b) + T1(i, a) * T1(j, b) - T1(i, b) * T1(j, a); };
+  auto mnef = [&](int m, int n, int e, int g) { return c.oovv[IDX4(m, n, e, g, o, v, v)]; };
+  auto mbef = [&](int m, int b, int e, int g) { return c.ovvv[IDX4(m, b, e, g, v, v, v)]; };
+  auto amef = [&](int a, int m, int e, int g) { return -mbef(m, a, e, g); };          // <am||ef> = -<ma||ef>
+  auto mbei = [&](int m, int b, int e, int i) { return c.ovvo[IDX4(m, b, e, i, v, v, o)]; };
+  auto mnei = [&](int m, int n, int e, int i) { return -c.ooov[IDX4(m, n, i, e, o, o, v)]; };   // <mn||ei> = -<mn||ie>
+  c.Wamef.assign((size_t)v * o * v * v, 0.0);
+#pragma omp parallel for collapse(2)
+  for (int a = 0; a < v; ++a)
+    for (int m = 0; m < o; ++m)
+      for (int e = 0; e < v; ++e)
+        for (int g = 0; g < v; ++g) {
+          double acc = amef(a, m, e, g);
+          for (int n = 0; n < o; ++n) acc -= T1(n, a) * mnef(n, m, e, g);
+          c.Wamef[IDX4(a, m, e, g, o, v, v)] = acc;
+        }
+  c.Wabef.assign((size_t)v * v * v * v, 0.0);
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int a = 0; a < v; ++a)
+    for (int b = 0; b < v; ++b)
+      for (int e = 0; e < v; ++e)
+        for (int g = 0; g < v; ++g) {
+          double acc = c.vvvv[IDX4(a, b, e, g, v, v, v)];
+          for (int m = 0; m < o; ++m) acc -= T1(m, b) * amef(a, m, e, g) - T1(m, a) * amef(b, m, e, g);
+          for (int m = 0; m < o; ++m)
+            for (int n = 0; n < o; ++n) acc += 0.5 * TAU(m, n, a, b) * mnef(m, n, e, g);
+          c.Wabef[IDX4(a, b, e, g, v, v, v)] = acc;
+        }
+  // the P(ab) pieces of W_abei as arrays in (a,b,e,i)
+  std::vector<double> tmp1((size_t)v * v * v * o, 0.0), tmp2((size_t)v * v * v * o, 0.0), par((size_t)o * v * v * o, 0.0);
+#pragma omp parallel for collapse(2)
+  for (int m = 0; m < o; ++m)
+    for (int b = 0; b < v; ++b)
+      for (int e = 0; e < v; ++e)
+        for (int i = 0; i < o; ++i) {
+          double acc = mbei(m, b, e, i);
+          for (int n = 0; n < o; ++n)
+            for (int g = 0; g < v; ++g) acc -= T2(n, i, b, g) * mnef(m, n, e, g);
+          par[IDX4(m, b, e, i, v, v, o)] = acc;
+        }
+#pragma omp parallel for collapse(2)
+  for (int a = 0; a < v; ++a)
+    for (int b = 0; b < v; ++b)
+      for (int e = 0; e < v; ++e)
+        for (int i = 0; i < o; ++i) {
+          double x1 = 0.0, x2 = 0.0;
+          for (int m = 0; m < o; ++m)
+            for (int g = 0; g < v; ++g) x1 += mbef(m, b, e, g) * T2(m, i, a, g);
+          for (int m = 0; m < o; ++m) x2 += T1(m, a) * par[IDX4(m, b, e, i, v, v, o)];
+          tmp1[IDX4(a, b, e, i, v, v, o)] = x1;
+          tmp2[IDX4(a, b, e, i, v, v, o)] = x2;
+        }
+  c.Wabei.assign((size_t)v * v * v * o, 0.0);
+#pragma omp parallel for collapse(2)
+  for (int a = 0; a < v; ++a)
+    for (int b = 0; b < v; ++b)
+      for (int e = 0; e < v; ++e)
+        for (int i = 0; i < o; ++i) {
+          double acc = c.vvvo[IDX4(a, b, e, i, v, v, o)];
+          for (int m = 0; m < o; ++m)
+            for (int n = 0; n < o; ++n) acc += 0.5 * mnei(m, n, e, i) * TAU(m, n, a, b);
+          for (int m = 0; m < o; ++m) acc -= c.Fme[(i64)m * v + e] * T2(m, i, a, b);
+          for (int g = 0; g < v; ++g) acc += c.Wabef[IDX4(a, b, e, g, v, v, v)] * T1(i, g);
+          acc -= tmp1[IDX4(a, b, e, i, v, v, o)] - tmp1[IDX4(b, a, e, i, v, v, o)];
+          acc -= tmp2[IDX4(a, b, e, i, v, v, o)] - tmp2[IDX4(b, a, e, i, v, v, o)];
+          c.Wabei[IDX4(a, b, e, i, v, v, o)] = acc;
+        }
+  c.has_ea = true;
+}
+
+// sigma_EA for one right-hand side.  y1 [v], y2 [o][v][v] (antisymmetric in a,b); s1, s2 same shapes.
+void sigma_ea_one(const Ctx& c, double omega, double eta, const cd* y1, const cd* y2, cd* s1, cd* s2) {
+  const int o = c.o, v = c.v;
+  const cd shift(omega, eta);
+  auto Y2 = [&](int j, int a, int b) { return y2[((i64)j * v + a) * v + b]; };
+  // w[k] = 1/2 sum_lcd <kl||cd> y2[l,c,d]
+  std::vector<cd> w(o);
+  for (int k = 0; k < o; ++k) {
+    cd acc = 0.0;
+    for (int l = 0; l < o; ++l)
+      for (int cc = 0; cc < v; ++cc)
+        for (int d = 0; d < v; ++d) acc += 0.5 * c.oovv[IDX4(k, l, cc, d, o, v, v)] * Y2(l, cc, d);
+    w[k] = acc;
+  }
+#pragma omp parallel for
+  for (int a = 0; a < v; ++a) {
+    cd acc = 0.0;
+    for (int cc = 0; cc < v; ++cc) acc += c.Fae[(i64)a * v + cc] * y1[cc];
+    for (int l = 0; l < o; ++l)
+      for (int d = 0; d < v; ++d) acc += c.Fme[(i64)l * v + d] * Y2(l, a, d);
+    for (int l = 0; l < o; ++l)
+      for (int cc = 0; cc < v; ++cc)
+        for (int d = 0; d < v; ++d) acc += 0.5 * c.Wamef[IDX4(a, l, cc, d, o, v, v)] * Y2(l, cc, d);
+    s1[a] = shift * y1[a] - acc;
+  }
+#pragma omp parallel for collapse(2) schedule(dynamic, 4)
+  for (int j = 0; j < o; ++j)
+    for (int a = 0; a < v; ++a)
+      for (int b = 0; b < v; ++b) {
+        cd acc = 0.0;
+        for (int cc = 0; cc < v; ++cc) acc += c.Wabei[IDX4(a, b, cc, j, v, v, o)] * y1[cc];
+        for (int cc = 0; cc < v; ++cc) acc += c.Fae[(i64)a * v + cc] * Y2(j, cc, b) - c.Fae[(i64)b * v + cc] * Y2(j, cc, a);
+        for (int l = 0; l < o; ++l) acc -= c.Fmi[(i64)l * o + j] * Y2(l, a, b);
+        for (int l = 0; l < o; ++l)
+          for (int d = 0; d < v; ++d)
+            acc += c.Wmbej[IDX4(l, b, d, j, v, v, o)] * Y2(l, a, d) - c.Wmbej[IDX4(l, a, d, j, v, v, o)] * Y2(l, b, d);
+        for (int cc = 0; cc < v; ++cc)
+          for (int d = 0; d < v; ++d) acc += 0.5 * c.Wabef[IDX4(a, b, cc, d, v, v, v)] * Y2(j, cc, d);
+        for (int k = 0; k < o; ++k) acc -= w[k] * c.t2[IDX4(k, j, a, b, o, v, v)];
+        s2[((i64)j * v + a) * v + b] = shift * Y2(j, a, b) - acc;
+      }
+}
+
+// ------------------------------------------------------------------------------------
+// GMRES(m) iteration shared by the IP system (Eq. 5) and the EA system (Eq. 6): Saad & Schultz 1986 (PAPER.md ref. 85;
+// PAPER.md:136-138), modified Gram-Schmidt Arnoldi in the plain Euclidean metric of the PACKED vector, complex Givens
+// rotations, stop when the rotated residual |g_{j+1}| <= tol * ||b||.  apply(z, Az) is the operator; x holds x0 on entry
+// and the iterate on exit.  Returns the number of operator applications; res = final relative residual (estimate).
+// hist (nullable): hist[k] = residual estimate after application k+1 (an output only).
+// ------------------------------------------------------------------------------------
+template <class Apply>
+int gmres_core(i64 n, Apply&& apply, const std::vector<cd>& b, std::vector<cd>& x, double tol, int m, int maxit, double& res_out,
+               double* hist, int nhist) {
+  auto dot = [&](const std::vector<cd>& a, const std::vector<cd>& bb) {
+    cd acc = 0.0;
+    for (i64 k = 0; k < n; ++k) acc += std::conj(a[k]) * bb[k];
+    return acc;
+  };
+  std::vector<cd> r, w;
+  const double bnorm = std::sqrt(std::real(dot(b, b)));
+  int napply = 0;
+  double res = 1.0;
+  while (napply < maxit) {
+    apply(x, w); ++napply;
+    r.resize(n);
+    for (i64 k = 0; k < n; ++k) r[k] = b[k] - w[k];
+    const double beta = std::sqrt(std::real(dot(r, r)));
+    res = beta / bnorm;
+    if (hist && napply - 1 < nhist) hist[napply - 1] = res;
+    if (res <= tol) break;
+    std::vector<std::vector<cd>> V(1, r);
+    for (auto& e : V[0]) e /= beta;
+    std::vector<std::vector<cd>> H(m + 1, std::vector<cd>(m, 0.0));
+    std::vector<cd> cs(m), sn(m), g(m + 1, 0.0);
+    g[0] = beta;
+    int j = 0;
+    for (; j < m && napply < maxit; ++j) {
+      apply(V[j], w); ++napply;
+      for (int k = 0; k <= j; ++k) {
+        H[k][j] = dot(V[k], w);
+        for (i64 q = 0; q < n; ++q) w[q] -= H[k][j] * V[k][q];
+      }
+      const double hn = std::sqrt(std::real(dot(w, w)));
+      H[j + 1][j] = hn;
+      for (int k = 0; k < j; ++k) {   // previous rotations
+        cd a = H[k][j], bb = H[k + 1][j];
+        H[k][j] = std::conj(cs[k]) * a + std::conj(sn[k]) * bb;
+        H[k + 1][j] = -sn[k] * a + cs[k] * bb;
+      }
+      {   // new rotation annihilating H[j+1][j]
+        cd a = H[j][j]; double bb = hn;
+        double den = std::sqrt(std::norm(a) + bb * bb);
+        cs[j] = a / den; sn[j] = bb / den;
+        H[j][j] = std::conj(cs[j]) * a + std::conj(sn[j]) * bb;
+        H[j + 1][j] = 0.0;
+        g[j + 1] = -sn[j] * g[j];
+        g[j] = std::conj(cs[j]) * g[j];
+      }
+      res = std::abs(g[j + 1]) / bnorm;
+      if (hist && napply - 1 < nhist) hist[napply - 1] = res;
+      if (res <= tol || hn == 0.0) { ++j; break; }
+      V.push_back(w);
+      for (auto& e : V.back()) e /= hn;
+    }
+    // back substitution and update
+    std::vector<cd> yv(j);
+    for (int k = j - 1; k >= 0; --k) {
+      cd acc = g[k];
+      for (int q = k + 1; q < j; ++q) acc -= H[k][q] * yv[q];
+      yv[k] = acc / H[k][k];
+    }
+    for (int k = 0; k < j; ++k)
+      for (i64 q = 0; q < n; ++q) x[q] += yv[k] * V[k][q];
+    if (res <= tol) break;
+  }
+  res_out = res;
+  return napply;
+}
+
 }  // namespace
 
 extern "C" {
 
 // mode bit 0: build the definition-form arrays (items 1-7; needs O(o v^3) memory);
-// mode bit 1: build the T1-dressed blocks for the row-sampled sigma.
+// mode bit 1: build the T1-dressed blocks for the row-sampled sigma;
+// mode bit 2 (with bit 0): build the EA intermediates W_amef, W_abef, W_abei (needs O(v^4) memory).
 void* orc_create(int o, int v, int Q, const double* fock, const double* T1, const double* T2p, const double* L1,
                  const double* L2p, const double* Lchol, int mode) {
   Ctx* c = new Ctx();
@@ -433,6 +648,7 @@ void* orc_create(int o, int v, int Q, const double* fock, const double* T1, cons
   c->T2p = T2p; c->L2p = L2p; c->L = Lchol;
   if (mode & 1) build_def(*c);
   if (mode & 2) build_dressed(*c);
+  if ((mode & 4) && c->has_def) build_ea(*c);
   return c;
 }
 void orc_destroy(void* h) { delete (Ctx*)h; }
@@ -453,6 +669,7 @@ i64 orc_get(void* h, const char* name, double* out) {
   if (n == "Fme") src = &c.Fme; else if (n == "Fmi") src = &c.Fmi; else if (n == "Fae") src = &c.Fae;
   else if (n == "Wmnij") src = &c.Wmnij; else if (n == "Wmnie") src = &c.Wmnie; else if (n == "Wmbej") src = &c.Wmbej;
   else if (n == "Wmbij") src = &c.Wmbij; else if (n == "oovv") src = &c.oovv; else if (n == "ft") src = &c.ft;
+  else if (n == "Wamef") src = &c.Wamef; else if (n == "Wabef") src = &c.Wabef; else if (n == "Wabei") src = &c.Wabei;
   if (!src) return -1;
   if (out) std::memcpy(out, src->data(), src->size() * sizeof(double));
   return (i64)src->size();
@@ -578,18 +795,12 @@ int orc_gmres_hist(void* h, int p, double omega, double eta, double tol, int m, 
     sigma_def_one(c, omega, eta, t1b.data(), t2b.data(), s1b.data(), s2b.data());
     pack(s1b.data(), s2b.data(), Az);
   };
-  auto dot = [&](const std::vector<cd>& a, const std::vector<cd>& b) {
-    cd acc = 0.0;
-    for (i64 k = 0; k < n; ++k) acc += std::conj(a[k]) * b[k];
-    return acc;
-  };
-  std::vector<cd> b, x(n, 0.0), r, w;
+  std::vector<cd> b, x(n, 0.0);
   {
     std::vector<cd> b1(o), b2(n2);
     orc_rhs(h, p, b1.data(), b2.data());
     pack(b1.data(), b2.data(), b);
   }
-  const double bnorm = std::sqrt(std::real(dot(b, b)));
   if (x0kind == 1) {
     const cd shift(omega, -eta);
     auto F = [&](int q) { return c.f[(i64)q * N + q]; };
@@ -599,61 +810,8 @@ int orc_gmres_hist(void* h, int p, double omega, double eta, double tol, int m, 
       for (int j = i + 1; j < o; ++j)
         for (int a = 0; a < v; ++a) { x[k] = b[k] / (shift + F(o + a) - F(i) - F(j)); ++k; }
   }
-  int napply = 0;
   double res = 1.0;
-  while (napply < maxit) {
-    apply(x, w); ++napply;
-    r.resize(n);
-    for (i64 k = 0; k < n; ++k) r[k] = b[k] - w[k];
-    const double beta = std::sqrt(std::real(dot(r, r)));
-    res = beta / bnorm;
-    if (hist && napply - 1 < nhist) hist[napply - 1] = res;
-    if (res <= tol) break;
-    std::vector<std::vector<cd>> V(1, r);
-    for (auto& e : V[0]) e /= beta;
-    std::vector<std::vector<cd>> H(m + 1, std::vector<cd>(m, 0.0));
-    std::vector<cd> cs(m), sn(m), g(m + 1, 0.0);
-    g[0] = beta;
-    int j = 0;
-    for (; j < m && napply < maxit; ++j) {
-      apply(V[j], w); ++napply;
-      for (int k = 0; k <= j; ++k) {
-        H[k][j] = dot(V[k], w);
-        for (i64 q = 0; q < n; ++q) w[q] -= H[k][j] * V[k][q];
-      }
-      const double hn = std::sqrt(std::real(dot(w, w)));
-      H[j + 1][j] = hn;
-      for (int k = 0; k < j; ++k) {   // previous rotations
-        cd a = H[k][j], bb = H[k + 1][j];
-        H[k][j] = std::conj(cs[k]) * a + std::conj(sn[k]) * bb;
-        H[k + 1][j] = -sn[k] * a + cs[k] * bb;
-      }
-      {   // new rotation annihilating H[j+1][j]
-        cd a = H[j][j]; double bb = hn;
-        double den = std::sqrt(std::norm(a) + bb * bb);
-        cs[j] = a / den; sn[j] = bb / den;
-        H[j][j] = std::conj(cs[j]) * a + std::conj(sn[j]) * bb;
-        H[j + 1][j] = 0.0;
-        g[j + 1] = -sn[j] * g[j];
-        g[j] = std::conj(cs[j]) * g[j];
-      }
-      res = std::abs(g[j + 1]) / bnorm;
-      if (hist && napply - 1 < nhist) hist[napply - 1] = res;
-      if (res <= tol || hn == 0.0) { ++j; break; }
-      V.push_back(w);
-      for (auto& e : V.back()) e /= hn;
-    }
-    // back substitution and update
-    std::vector<cd> yv(j);
-    for (int k = j - 1; k >= 0; --k) {
-      cd acc = g[k];
-      for (int q = k + 1; q < j; ++q) acc -= H[k][q] * yv[q];
-      yv[k] = acc / H[k][k];
-    }
-    for (int k = 0; k < j; ++k)
-      for (i64 q = 0; q < n; ++q) x[q] += yv[k] * V[k][q];
-    if (res <= tol) break;
-  }
+  const int napply = gmres_core(n, apply, b, x, tol, m, maxit, res, hist, nhist);
   unpack(x, x1out, x2out);
   *relres = res;
   return napply;
@@ -889,6 +1047,140 @@ int orc_sigma_rows(void* h, int nrhs, const double* omega, double eta, const cd*
     }
   }
   return 0;
+}
+
+// ------------------------------------------------------------------------------------
+// EA / advanced part: C entry points (Eq. 6; second terms of Eq. 7-8).
+// Y1 [nrhs][v], Y2 [nrhs][o][v][v] (index order j, a, b; antisymmetric in a,b), complex interleaved.
+// ------------------------------------------------------------------------------------
+int orc_sigma_ea(void* h, int nrhs, const double* omega, double eta, const cd* Y1, const cd* Y2, cd* S1, cd* S2) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.has_ea) return -1;
+  const i64 n2 = (i64)c.o * c.v * c.v;
+  for (int r = 0; r < nrhs; ++r) sigma_ea_one(c, omega[r], eta, Y1 + (i64)r * c.v, Y2 + r * n2, S1 + (i64)r * c.v, S2 + r * n2);
+  return 0;
+}
+
+// Right-hand side of Eq. 6: projections of abar_q^+ |Phi> on the 1p and 2p1h determinants.
+//   q = o+c virtual: b1[a] = delta_ac, b2 = 0;   q = k occupied: b1[a] = -t[k,a], b2[j,a,b] = -t[k,j,a,b].
+int orc_rhs_ea(void* h, int q, cd* b1, cd* b2) {
+  Ctx& c = *(Ctx*)h;
+  const int o = c.o, v = c.v;
+  if (q < 0 || q >= c.N) return -1;
+  for (int a = 0; a < v; ++a) b1[a] = 0.0;
+  for (i64 k = 0; k < (i64)o * v * v; ++k) b2[k] = 0.0;
+  if (q >= o) { b1[q - o] = 1.0; return 0; }
+  for (int a = 0; a < v; ++a) b1[a] = -c.t1[(i64)q * v + a];
+  for (int j = 0; j < o; ++j)
+    for (int a = 0; a < v; ++a)
+      for (int b = 0; b < v; ++b) b2[((i64)j * v + a) * v + b] = -t2p_at(c, q, j, a, b);
+  return 0;
+}
+
+// Bra vector of the second term of Eq. 7-8: c_p[nu] = <Phi|(1 + Lambda1 + Lambda2) abar_p tau_nu|Phi>, real.
+//   p = k occupied : c1[a] = -l[k,a];  c2[j,a,b] = -l[k,j,a,b]
+//   p = o+e virtual: c1[a] = delta_ea - sum_i l[i,a] t[i,e] - 1/2 sum_ijb l[i,j,a,b] t[i,j,e,b]
+//                    c2[j,a,b] = delta_ea l[j,b] - delta_eb l[j,a] - sum_i t[i,e] l[i,j,a,b]
+// G^A_pq = sum_a c1[a] y1[a] + sum_{j, a<b} c2[j,a,b] y2[j,a,b].
+int orc_bra_ea(void* h, int p, double* c1, double* c2) {
+  Ctx& c = *(Ctx*)h;
+  const int o = c.o, v = c.v;
+  if (p < 0 || p >= c.N) return -1;
+  if (p < o) {
+    for (int a = 0; a < v; ++a) c1[a] = -c.l1[(i64)p * v + a];
+    for (int j = 0; j < o; ++j)
+      for (int a = 0; a < v; ++a)
+        for (int b = 0; b < v; ++b) c2[((i64)j * v + a) * v + b] = -l2p_at(c, p, j, a, b);
+    return 0;
+  }
+  const int e = p - o;
+#pragma omp parallel for
+  for (int a = 0; a < v; ++a) {
+    double acc = (a == e) ? 1.0 : 0.0;
+    for (int i = 0; i < o; ++i) acc -= c.l1[(i64)i * v + a] * c.t1[(i64)i * v + e];
+    for (int i = 0; i < o; ++i)
+      for (int j = 0; j < o; ++j)
+        for (int b = 0; b < v; ++b) acc -= 0.5 * l2p_at(c, i, j, a, b) * t2p_at(c, i, j, e, b);
+    c1[a] = acc;
+  }
+#pragma omp parallel for collapse(2)
+  for (int j = 0; j < o; ++j)
+    for (int a = 0; a < v; ++a)
+      for (int b = 0; b < v; ++b) {
+        double acc = 0.0;
+        if (a == e) acc += c.l1[(i64)j * v + b];
+        if (b == e) acc -= c.l1[(i64)j * v + a];
+        for (int i = 0; i < o; ++i) acc -= c.t1[(i64)i * v + e] * l2p_at(c, i, j, a, b);
+        c2[((i64)j * v + a) * v + b] = acc;
+      }
+  return 0;
+}
+
+void orc_bra_dot_ea(void* h, const double* c1, const double* c2, const cd* y1, const cd* y2, cd* out) {
+  Ctx& c = *(Ctx*)h;
+  const int o = c.o, v = c.v;
+  cd acc = 0.0;
+  for (int a = 0; a < v; ++a) acc += c1[a] * y1[a];
+  for (int j = 0; j < o; ++j)
+    for (int a = 0; a < v; ++a)
+      for (int b = a + 1; b < v; ++b) acc += c2[((i64)j * v + a) * v + b] * y2[((i64)j * v + a) * v + b];
+  *out = acc;
+}
+
+// GMRES(m) for Eq. 6 with target q, packed vector z = (y1[a], y2[j, a<b]) (j slowest).
+// x0kind 1: y0 = b / (omega + i eta - d), d_a = f_aa, d_jab = f_aa + f_bb - f_jj (zeroth order of Hbar on 1p / 2p1h).
+int orc_gmres_ea(void* h, int q, double omega, double eta, double tol, int m, int maxit, int x0kind, cd* y1out, cd* y2out,
+                 double* relres, double* hist, int nhist) {
+  Ctx& c = *(Ctx*)h;
+  if (!c.has_ea) return -1;
+  const int o = c.o, v = c.v, N = c.N;
+  const i64 n2 = (i64)o * v * v, n = v + (i64)o * c.ntri;
+  auto pack = [&](const cd* a1, const cd* a2, std::vector<cd>& z) {
+    z.resize(n);
+    for (int a = 0; a < v; ++a) z[a] = a1[a];
+    i64 k = v;
+    for (int j = 0; j < o; ++j)
+      for (int a = 0; a < v; ++a)
+        for (int b = a + 1; b < v; ++b) z[k++] = a2[((i64)j * v + a) * v + b];
+  };
+  auto unpack = [&](const std::vector<cd>& z, cd* a1, cd* a2) {
+    for (int a = 0; a < v; ++a) a1[a] = z[a];
+    for (i64 k = 0; k < n2; ++k) a2[k] = 0.0;
+    i64 k = v;
+    for (int j = 0; j < o; ++j)
+      for (int a = 0; a < v; ++a)
+        for (int b = a + 1; b < v; ++b) {
+          a2[((i64)j * v + a) * v + b] = z[k];
+          a2[((i64)j * v + b) * v + a] = -z[k];
+          ++k;
+        }
+  };
+  std::vector<cd> t1b(v), t2b(n2), s1b(v), s2b(n2);
+  auto apply = [&](const std::vector<cd>& z, std::vector<cd>& Az) {
+    unpack(z, t1b.data(), t2b.data());
+    sigma_ea_one(c, omega, eta, t1b.data(), t2b.data(), s1b.data(), s2b.data());
+    pack(s1b.data(), s2b.data(), Az);
+  };
+  std::vector<cd> b, x(n, 0.0);
+  {
+    std::vector<cd> b1(v), b2(n2);
+    orc_rhs_ea(h, q, b1.data(), b2.data());
+    pack(b1.data(), b2.data(), b);
+  }
+  if (x0kind == 1) {
+    const cd shift(omega, eta);
+    auto F = [&](int r) { return c.f[(i64)r * N + r]; };
+    for (int a = 0; a < v; ++a) x[a] = b[a] / (shift - F(o + a));
+    i64 k = v;
+    for (int j = 0; j < o; ++j)
+      for (int a = 0; a < v; ++a)
+        for (int bb = a + 1; bb < v; ++bb) { x[k] = b[k] / (shift - F(o + a) - F(o + bb) + F(j)); ++k; }
+  }
+  double res = 1.0;
+  const int napply = gmres_core(n, apply, b, x, tol, m, maxit, res, hist, nhist);
+  unpack(x, y1out, y2out);
+  *relres = res;
+  return napply;
 }
 
 }  // extern "C"

@@ -34,8 +34,8 @@ def antisym_integrals(L):
     return g - g.transpose(0, 1, 3, 2)
 
 
-def brute_force(o, v, f, L, t1, t2, l1, l2):
-    """returns H_IP [n,n], b [N,n], c [N,n] in the packed basis (1h then (i<j,a) row-major)."""
+def operators(o, v, f, L, t1, t2, l1, l2):
+    """Jordan-Wigner matrices of everything the projections below need: (a, ad, phi, Hbar, Lam, emT, eT)."""
     N = o + v
     a = jw_annihilators(N)
     ad = [x.T for x in a]
@@ -73,6 +73,14 @@ def brute_force(o, v, f, L, t1, t2, l1, l2):
                     Lam += 0.25 * l2[i, j, aa, bb] * ad[i] @ ad[j] @ a[o + bb] @ a[o + aa]
     eT, emT = expm(T), expm(-T)
     Hbar = emT @ HN @ eT
+    return a, ad, phi, Hbar, Lam, emT, eT
+
+
+def brute_force(o, v, f, L, t1, t2, l1, l2, ops=None):
+    """returns H_IP [n,n], b [N,n], c [N,n] in the packed basis (1h then (i<j,a) row-major)."""
+    N = o + v
+    a, ad, phi, Hbar, Lam, emT, eT = ops if ops is not None else operators(o, v, f, L, t1, t2, l1, l2)
+    dim = 2 ** N
     taus = [a[i] for i in range(o)]
     for i in range(o):
         for j in range(i + 1, o):
@@ -94,3 +102,36 @@ def brute_force(o, v, f, L, t1, t2, l1, l2):
             bs[p, mu] = phi @ taus[mu].T @ abar @ phi
             cs[p, mu] = phi @ onepl @ adbar @ taus[mu] @ phi
     return HIP, bs, cs
+
+
+def brute_force_ea(o, v, f, L, t1, t2, l1, l2, ops=None):
+    """Advanced (electron-attached) part, Eq. 4, Eq. 6, second terms of Eq. 7-8:
+        basis  tau_a = a+_a, tau_jab = a+_a a+_b a_j (a<b)          (Eq. 4 operator order)
+        Hbar_EA[mu,nu] = <Phi| tau_mu^+ [Hbar, tau_nu] |Phi>        (connected action, reading 5)
+        b_q[mu] = <Phi| tau_mu^+ exp(-T) a+_q exp(T) |Phi>          (Eq. 6 rhs)
+        c_p[nu] = <Phi| (1+Lambda) exp(-T) a_p exp(T) tau_nu |Phi>   (Eq. 7 second term)
+    returns H_EA [n,n], b [N,n], c [N,n] in the packed basis (1p, then (j, a<b) row-major: j slowest)."""
+    N = o + v
+    a, ad, phi, Hbar, Lam, emT, eT = ops if ops is not None else operators(o, v, f, L, t1, t2, l1, l2)
+    dim = 2 ** N
+    taus = [ad[o + aa] for aa in range(v)]
+    for j in range(o):
+        for aa in range(v):
+            for bb in range(aa + 1, v):
+                taus.append(ad[o + aa] @ ad[o + bb] @ a[j])
+    n = len(taus)
+    HEA = np.zeros((n, n))
+    for mu in range(n):
+        bra = phi @ taus[mu].T
+        for nu in range(n):
+            HEA[mu, nu] = bra @ (Hbar @ taus[nu] - taus[nu] @ Hbar) @ phi
+    bs = np.zeros((N, n))
+    cs = np.zeros((N, n))
+    onepl = np.eye(dim) + Lam
+    for p in range(N):
+        abar = emT @ a[p] @ eT
+        adbar = emT @ ad[p] @ eT
+        for mu in range(n):
+            bs[p, mu] = phi @ taus[mu].T @ adbar @ phi
+            cs[p, mu] = phi @ onepl @ abar @ taus[mu] @ phi
+    return HEA, bs, cs

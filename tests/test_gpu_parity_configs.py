@@ -133,6 +133,53 @@ def test_config1_solve_residual_rows_and_G():
     g.gfcc_destroy(h)
 
 
+def test_config2_fixed_step_solve_vs_oracle():
+    """config 2 in the mode bench.py --config 2 times (fixed Arnoldi steps; the k-step iterate is unique, reading 19):
+    the GPU's X after k steps is checked WITHOUT the GPU's own sigma -- sampled rows of b - sigma_oracle(X) equal the rows of
+    the GPU's residual vector b - sigma_gpu(X), whose norm equals the residual the device-side Givens recurrence reports --
+    and G equals the oracle's bra vectors dotted with X (G1-G6 at full config-2 size)."""
+    g, c, s, h, orc = _setup(2)
+    o, v, eta = c["o"], c["v"], c["eta"]
+    plist = [o - 1, o - 2, o + 3]
+    ws = np.array([c["wlo"], c["whi"]])
+    k = 4
+    g.gfcc_set_option(h, "gmres_fixed", k)
+    G, X1, X2 = g.gfcc_solve_ip(h, plist, ws, eta, c["tol"], return_x=True)
+    g.gfcc_set_option(h, "gmres_fixed", 0)
+    nr = len(plist) * len(ws)
+    rel, its = g.gfcc_get_residuals(h, nr)
+    assert (its == k).all()
+    wr = np.array([ws[iw] for ip in range(len(plist)) for iw in range(len(ws))])
+    S1, S2 = g.gfcc_sigma_ip(h, wr, eta, X1, X2)
+    X1h, X2h, S1h, S2h = X1.cpu().numpy(), X2.cpu().numpy(), S1.cpu().numpy(), S2.cpu().numpy()
+    trip = _triples(o, v, 5, 11)
+    s1rows = [0, o - 1]
+    R1, R2 = orc.sigma_rows(wr, eta, X1h, X2h, s1rows, trip)
+    for r in range(nr):
+        b1, b2 = orc.rhs(plist[r // len(ws)])
+        bn = np.linalg.norm(orc.pack(b1, b2))
+        res_gpu = orc.pack(b1 - S1h[r], b2 - S2h[r])
+        rn = np.linalg.norm(res_gpu)
+        assert abs(rn / bn / rel[r] - 1) < 1e-8, (r, rn / bn, rel[r])          # Givens estimate = true residual norm
+        hist = g.gfcc_get_residual_history(h, r)
+        assert len(hist) == k + 1 and (np.diff(hist) <= 0).all()
+        # residual rows from the ORACLE's sigma of the GPU's X against the GPU's residual vector
+        o1 = b1[s1rows] - R1[:, r]
+        o2 = np.array([b2[i, j, a] for (i, j, a) in trip]) - R2[:, r]
+        g1 = (b1 - S1h[r])[s1rows]
+        g2 = np.array([(b2 - S2h[r])[i, j, a] for (i, j, a) in trip])
+        scale = max(np.abs(S2h[r]).max(), np.abs(S1h[r]).max())
+        assert np.abs(o1 - g1).max() <= TOL_SIGMA * scale and np.abs(o2 - g2).max() <= TOL_SIGMA * scale
+    for iq, q in enumerate(plist):
+        c1, c2 = orc.bra(q)
+        for ip in range(len(plist)):
+            for iw in range(len(ws)):
+                r = ip * len(ws) + iw
+                ref = orc.bra_dot(c1, c2, X1h[r], X2h[r])
+                assert abs(G[iw, ip, iq] - ref) <= TOL_G * max(abs(ref), np.abs(G[iw]).max())
+    g.gfcc_destroy(h)
+
+
 # ---------------------------------------------------------------------------------------------------------------
 # Configs 3 and 4 (the benched config): the oracle needs 30 / 115 GB of host memory, minutes of dressing and 20-90 s per sigma2
 # row, so its values are STORED: tests/golden/config{3,4}_rows.npz, written by tests/golden/make_rows.py, which imports only
