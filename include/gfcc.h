@@ -137,6 +137,25 @@ int gfcc_get_residual_history(gfcc_handle h, int rhs, int cap, double* hist, int
  * Gout host or device.  Linear in X: gfcc_solve_ip's G is this map applied to the solutions.  Synchronous.             */
 int gfcc_assemble_g(gfcc_handle h, int nrhs, const void* X1, const void* X2, int nq, const int* q, void* Gout);
 
+/* ---- EA / advanced part (Eq. 4, Eq. 6, second terms of Eq. 7-8) ----
+ * Y_q = sum_a y1[a] a+_a + sum_{j, a<b} y2[j,a,b] a+_a a+_b a_j solves (omega - Hbar_N + i eta) Y_q |Phi> = abar_q^+ |Phi>, and
+ * G^A_pq = <Phi|(1+Lambda1+Lambda2) abar_p (Y_q1 + Y_q2)|Phi> is the second term of Eq. 8 (the full GFCCSD matrix element is
+ * gfcc_solve_ip's G + this G^A).  Working equations: DESIGN.md section 6.8.  Vector layouts: Y1 complex [nrhs][v],
+ * Y2 complex [nrhs][o][v][v] with index order (j, a, b), antisymmetric in (a, b) (precondition for inputs, guaranteed for outputs).
+ * The first EA call on a handle builds the stored intermediate W_abcj (o v^3 / 2 doubles: this part is meant for sizes where
+ * that fits, BASELINE.json configs 0-1) -- GFCC_ENOMEM otherwise.
+ *   gfcc_sigma_ea      sigma_r = (omega[r] + i eta) Y_r - Hbar Y_r,  r < nrhs; omega [host]; asynchronous like gfcc_sigma_ip
+ *   gfcc_solve_ea(_x)  batched GMRES (the solver of gfcc_solve_ip: CGS2, device Givens, compaction, refill, same options and
+ *                      statistics) for every (q = p[iq], omega[iw]), tasks r = iq*nw + iw, and
+ *                      G[iw][ip][iq] = G^A_{p[ip], p[iq]}(omega[iw])  complex [nw][np][np] (host or device);
+ *                      Y1out/Y2out (nullable, device) receive the solutions in task order
+ *   gfcc_assemble_g_ea Gout[r][ip] = c_{p[ip]} . Y_r for caller-provided vectors (complex [nrhs][np], host or device)      */
+int gfcc_sigma_ea(gfcc_handle h, int nrhs, const double* omega, double eta, const void* Y1, const void* Y2, void* S1, void* S2);
+int gfcc_solve_ea(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol, void* G);
+int gfcc_solve_ea_x(gfcc_handle h, int np, const int* p, int nw, const double* omega, double eta, double tol, void* G,
+                    void* Y1out, void* Y2out);
+int gfcc_assemble_g_ea(gfcc_handle h, int nrhs, const void* Y1, const void* Y2, int np, const int* p, void* Gout);
+
 /* Copy a named intermediate to a caller buffer (device pointer, FP64), for parity tests:
  *   "Fme" [o][v], "Fmi" [o][o], "Fae" [v][v], "Wmnij" packed [npair(i<j)][npair(m<n)],
  *   "Wmbij" packed [npair(i<j)][v][o] holding W_mbij[m,a,j,i] at [pair(i,j)][a][m], "D" [o][o],

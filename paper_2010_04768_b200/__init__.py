@@ -25,7 +25,7 @@ EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip"
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_residual_history", "gfcc_assemble_g",
            "gfcc_get_intermediate", "gfcc_last_error",
            "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
-           "gfcc_mor_get", "gfcc_spectral_adaptive"]
+           "gfcc_mor_get", "gfcc_spectral_adaptive", "gfcc_sigma_ea", "gfcc_solve_ea", "gfcc_solve_ea_x", "gfcc_assemble_g_ea"]
 
 
 class GfccError(RuntimeError):
@@ -60,6 +60,10 @@ def lib():
     L.gfcc_get_residual_history.argtypes = [vp, ci, ci, dp, ip]
     L.gfcc_assemble_g.argtypes = [vp, ci, vp, vp, ci, ip, vp]
     L.gfcc_get_intermediate.argtypes = [vp, ctypes.c_char_p, vp]
+    L.gfcc_sigma_ea.argtypes = [vp, ci, dp, cd, vp, vp, vp, vp]
+    L.gfcc_solve_ea.argtypes = [vp, ci, ip, ci, dp, cd, cd, vp]
+    L.gfcc_solve_ea_x.argtypes = [vp, ci, ip, ci, dp, cd, cd, vp, vp, vp]
+    L.gfcc_assemble_g_ea.argtypes = [vp, ci, vp, vp, ci, ip, vp]
     L.gfcc_get_intermediate.restype = cll
     L.gfcc_last_error.argtypes = [vp]
     L.gfcc_last_error.restype = ctypes.c_char_p
@@ -323,6 +327,52 @@ def gfcc_probe_fp64_peak(iters=20000, reps=5, stream=0):
     if rc != GFCC_OK:
         raise GfccError(rc, "gfcc_probe_fp64_peak failed")
     return out.value
+
+
+# ---- EA / advanced part (Eq. 6; second terms of Eq. 7-8) ------------------------------------------
+def gfcc_sigma_ea(h, omega, eta, Y1, Y2, S1=None, S2=None):
+    """Y1 [nrhs,v], Y2 [nrhs,o,v,v] complex128 CUDA tensors -> (S1, S2) = (omega + i eta) Y - Hbar Y."""
+    torch = _torch()
+    c128 = torch.complex128
+    nrhs = Y1.shape[0]
+    if Y1.numel() != nrhs * h.v or Y2.numel() != nrhs * h.o * h.v * h.v:
+        raise GfccError(GFCC_EINVAL, "Y1/Y2 shape mismatch")
+    if S1 is None:
+        S1 = torch.empty_like(Y1)
+    if S2 is None:
+        S2 = torch.empty_like(Y2)
+    om, omp = _omega(omega, nrhs)
+    _check(h, lib().gfcc_sigma_ea(h.ptr, nrhs, omp, float(eta), _dev(Y1, c128), _dev(Y2, c128), _dev(S1, c128), _dev(S2, c128)))
+    return S1, S2
+
+
+def gfcc_solve_ea(h, p, omega, eta, tol, return_y=False, allow_noconv=False):
+    """advanced part: G^A [nw, np, np] (host numpy); return_y: also Y1 [np*nw, v], Y2 [np*nw, o, v, v] (task r = iq*nw + iw)."""
+    torch = _torch()
+    pa = np.ascontiguousarray(p, dtype=np.int32)
+    npn, nw = len(pa), len(np.atleast_1d(omega))
+    om, omp = _omega(np.atleast_1d(omega), nw)
+    G = np.empty((nw, npn, npn), dtype=np.complex128)
+    allow = (GFCC_ENOCONV,) if allow_noconv else ()
+    pp = pa.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+    if return_y:
+        Y1 = torch.empty((npn * nw, h.v), dtype=torch.complex128, device="cuda")
+        Y2 = torch.empty((npn * nw, h.o, h.v, h.v), dtype=torch.complex128, device="cuda")
+        _check(h, lib().gfcc_solve_ea_x(h.ptr, npn, pp, nw, omp, float(eta), float(tol), G.ctypes.data,
+                                        ctypes.c_void_p(Y1.data_ptr()), ctypes.c_void_p(Y2.data_ptr())), allow)
+        return G, Y1, Y2
+    _check(h, lib().gfcc_solve_ea(h.ptr, npn, pp, nw, omp, float(eta), float(tol), G.ctypes.data), allow)
+    return G
+
+
+def gfcc_assemble_g_ea(h, Y1, Y2, p):
+    torch = _torch()
+    pa = np.ascontiguousarray(p, dtype=np.int32)
+    nrhs = Y1.shape[0]
+    G = np.empty((nrhs, len(pa)), dtype=np.complex128)
+    _check(h, lib().gfcc_assemble_g_ea(h.ptr, nrhs, _dev(Y1, torch.complex128), _dev(Y2, torch.complex128), len(pa),
+                                       pa.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), G.ctypes.data))
+    return G
 
 
 # ---- model-order reduction (PAPER.md:110-126 Eq. 9-10; Alg. 1 lines 18-21) -----------------------------------

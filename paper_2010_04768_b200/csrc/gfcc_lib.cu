@@ -26,6 +26,7 @@
 #include "gfcc_probe.cuh"
 #include "gfcc_mor.cuh"
 #include "gfcc_ozaki.cuh"
+#include "gfcc_ea.cuh"
 
 using namespace gfcc;
 
@@ -39,7 +40,12 @@ struct NvtxRange {
 
 static thread_local std::string g_create_error;
 
+struct EaState;   // EA / advanced part (gfcc_ea_host.inl), created on first use
+static void ea_destroy(struct gfcc_ctx* h);
+static void ea_release_ws(struct gfcc_ctx* h);
+
 struct gfcc_ctx {
+  EaState* ea = nullptr;
   int o = 0, v = 0, Q = 0, N = 0;
   long long npair = 0, ntri = 0, nvec = 0;   // nvec = o + npair*v (rows of an internal vector)
   cudaStream_t stream = 0;
@@ -798,6 +804,7 @@ extern "C" int gfcc_destroy(gfcc_handle h) {
   cudaStreamSynchronize(h->stream);
   free_side_streams(h);
   solve_free(h->sw);
+  ea_destroy(h);
   for (void* p : h->allocs) cudaFree(p);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   delete h;
@@ -822,7 +829,7 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "x0" && (val == 0 || val == 1)) h->opt_x0 = val;
   else if (k == "panel_bytes" && val > 0) { h->opt_panel_bytes = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
-  else if (k == "release_workspace") { cudaStreamSynchronize(h->stream); if (h->ws_nrhs) free_workspace(h); solve_free(h->sw); }
+  else if (k == "release_workspace") { cudaStreamSynchronize(h->stream); if (h->ws_nrhs) free_workspace(h); solve_free(h->sw); ea_release_ws(h); }
   else if (k == "compact" && val <= 1) h->opt_compact = val;
   else if (k == "gmres_poll" && val >= 0) h->opt_poll = std::floor(val);
   else if (k == "overlap" && (val == 0 || val == 1)) { h->opt_overlap = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
@@ -1085,9 +1092,41 @@ extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, cons
     SigmaFn apply = [&](int nrhs, const double* d_omega, const double* xin, double* sout) -> int {
       return sigma_internal(h, nrhs, d_omega, eta, xin, sout);
     };
+    cudaStream_t st = h->stream;
+    SolveHooks hooks;
+    // G1: b_p and the zeroth-order guess for the batch columns [c0, A)
+    hooks.init = [&](double* b, double* x, int A, int c0, const int* p_col, const double* omega_col, double* nl) -> int {
+      const long long tot = h->nvec * (A - c0);
+      k_build_rhs<<<nblk(tot, 256, 148LL * 16), 256, 0, st>>>(b, p_col, h->t1, h->T2p, h->o, h->v, A, h->nvec, c0);
+      k_x0<<<(unsigned)(h->npair + 1), 256, 0, st>>>(x, b, omega_col, eta, h->fdiag, h->o, h->v, A, cfg.x0, c0);
+      *nl += 2;
+      return cudaGetLastError() == cudaSuccess ? 0 : GFCC_ECUDA;
+    };
+    // G6: g = Lambda2 . X2 and G_pq for the retired columns; optional X output in the C-ABI layout
+    hooks.finish = [&](const double* xr, int ld, int nret, const int* ret_row, double* nl) -> int {
+      SolveWs& s = h->sw;
+      const int Nc = 2 * ld;
+      dim3 grid((2 * nret + LG_CC - 1) / LG_CC, s.g_blocks);
+      static bool attr_set = false;
+      if (!attr_set) { cudaFuncSetAttribute(k_lambda2_g, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_set = true; }
+      k_lambda2_g<<<grid, 32 * LG_WARPS, lambda2_g_smem_bytes(h->v), st>>>(s.gpart, h->L2p, xr, h->o, h->v, Nc, h->npair);
+      const long long n = (long long)h->v * Nc;
+      k_g_reduce<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(s.gvec, s.gpart, s.g_blocks, n);
+      dim3 gg(np, nret);
+      k_assemble_G<<<gg, 256, 0, st>>>((double2*)Gq, dq, np, xr, s.gvec, h->D, h->t1, h->l1, h->o, h->v, ld, ret_row);
+      *nl += 3;
+      if (X1out && X2out) {
+        dim3 blk(32, 8), g2((unsigned)((h->nvec + 31) / 32), (unsigned)((nret + 31) / 32));
+        k_vec_to_abi<<<g2, blk, 0, st>>>((double2*)X1out, (double2*)X2out, xr, h->o, h->v, nret, ld, ret_row);
+        const long long tot = (long long)nret * h->o * h->v;
+        k_zero_diag<<<(unsigned)std::min<long long>(4096, (tot + 255) / 256), 256, 0, st>>>((double2*)X2out, h->o, h->v, nret, ret_row);
+        *nl += 2;
+      }
+      return cudaGetLastError() == cudaSuccess ? 0 : GFCC_ECUDA;
+    };
     std::string err;
     double nlaunch = 0;
-    int rc = solve_run(h->sw, cfg, tasks, apply, (double2*)Gq, dq, np, (double*)X1out, (double*)X2out, &h->last_hist, &nlaunch, err);
+    int rc = solve_run(h->sw, cfg, tasks, apply, hooks, &h->last_hist, &nlaunch, err);
     h->st_kernel_launches += nlaunch;
     if (rc == GFCC_ENOCONV) rc_final = GFCC_ENOCONV;
     else if (rc != GFCC_OK) { h->err = err; rc_final = rc; break; }
@@ -1173,5 +1212,6 @@ extern "C" int gfcc_assemble_g(gfcc_handle h, int nrhs, const void* X1, const vo
   return rc;
 }
 
+#include "gfcc_ea_host.inl"
 #include "gfcc_mor_host.inl"
 #include "gfcc_workflow_host.inl"

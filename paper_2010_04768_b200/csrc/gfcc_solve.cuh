@@ -384,7 +384,7 @@ static int solve_alloc(SolveWs& s, const SolveCfg& c, int mcap, std::string& err
   S_TRY(s_alloc(s, &s.xr, vecel, err)); S_TRY(s_alloc(s, &s.spare, vecel, err));
   s.dot_blocks = (int)std::min<long long>(592, std::max<long long>(1, c.nvec / 64));
   s.g_blocks = (int)std::min<long long>(296, c.npair);
-  s.histcap = std::min(std::max(c.maxit, c.fixed) + 2, 8192);
+  s.histcap = 8192;   // residual-history entries kept per right-hand side
   S_TRY(s_alloc(s, &s.H, (long long)(mcap + 2) * nr, err));
   S_TRY(s_alloc(s, &s.R, (long long)mcap * (mcap + 1) * nr, err));
   S_TRY(s_alloc(s, &s.cs, (long long)mcap * nr, err));
@@ -399,7 +399,7 @@ static int solve_alloc(SolveWs& s, const SolveCfg& c, int mcap, std::string& err
   S_TRY(s_alloc(s, &s.stat, 3LL * nr, err));
   S_TRY(s_alloc(s, &s.slot_col, nr, err)); S_TRY(s_alloc(s, &s.p_col, nr, err));
   S_TRY(s_alloc(s, &s.map, nr, err)); S_TRY(s_alloc(s, &s.ret_row, nr, err));
-  S_TRY(s_alloc(s, &s.gvec, (long long)c.v * 2 * nr, err));
+  S_TRY(s_alloc(s, &s.gvec, (long long)std::max(c.o, c.v) * 2 * nr, err));
   S_TRY(s_alloc(s, &s.gpart, (long long)s.g_blocks * c.v * 2 * nr, err));
   S_TRY(s_alloc(s, &s.vptr, mcap + 3, err));
   return 0;
@@ -410,8 +410,7 @@ static int solve_alloc(SolveWs& s, const SolveCfg& c, int mcap, std::string& err
 // different gmres_fixed takes effect without reallocation).  Nothing is committed unless every allocation succeeded.
 inline int solve_prepare(SolveWs& s, const SolveCfg& c, std::string& err) {
   const int want = c.fixed > 0 ? c.fixed : c.m;
-  const int histwant = std::min(std::max(c.maxit, c.fixed) + 2, 8192);
-  if (s.cap == c.batch && s.nvec == c.nvec && s.mcap >= want && s.histcap >= histwant && !s.V.empty()) {
+  if (s.cap == c.batch && s.nvec == c.nvec && s.mcap >= want && !s.V.empty()) {
     s.m_run = want;
     return 0;
   }
@@ -434,11 +433,19 @@ struct SolveTask {
 
 // sigma(nrhs, d_omega, xin, sout): batched sigma on internal vectors with nrhs active columns (0 or a GFCC error code)
 typedef std::function<int(int, const double*, const double*, double*)> SigmaFn;
+// The solver core is agnostic of what a vector row means (IP: 1h + 2h1p rows, Eq. 5; EA: 1p + 2p1h rows, Eq. 6).  Two hooks
+// supply the problem-specific pieces; both enqueue on the solver's stream and return 0 or a negative error code:
+//   init(b, x, A, c0, p_col, omega_col): right-hand sides and initial guesses of the active columns [c0, A) (row stride A)
+//   finish(xr, ld, nret, ret_row)      : G assembly (and optional X output) of the first nret columns of the retirement buffer
+//                                        xr (row stride ld complex columns); column r belongs to task ret_row[r] (device)
+struct SolveHooks {
+  std::function<int(double*, double*, int, int, const int*, const double*, double*)> init;
+  std::function<int(const double*, int, int, const int*, double*)> finish;
+};
 
 struct SolveRun {
-  SolveWs& s; const SolveCfg& c; const SigmaFn& sigma; std::string& err; double* nlaunch;
+  SolveWs& s; const SolveCfg& c; const SigmaFn& sigma; const SolveHooks& hooks; std::string& err; double* nlaunch;
   std::vector<SolveTask>& tasks;
-  double2* Gq; const int* qlist; int nq; double* X1out; double* X2out;
   std::vector<std::vector<double>>* hist_out;
   cudaStream_t st;
   int B, A = 0, nret = 0;
@@ -499,26 +506,12 @@ struct SolveRun {
   int* d_jstop() { return s.stat + B; }
   int* d_age() { return s.stat + 2 * B; }
 
-  // G assembly + X output of the retirement buffer, then empty it
+  // G assembly + X output of the retirement buffer (problem-specific hook), then empty it
   int flush() {
     if (nret == 0) return 0;
     S_CUDA(cudaMemcpyAsync(s.ret_row, ret_task.data(), nret * sizeof(int), cudaMemcpyHostToDevice, st));
-    const int Nc = 2 * B;
-    dim3 grid((2 * nret + LG_CC - 1) / LG_CC, s.g_blocks);
-    const size_t smem = lambda2_g_smem_bytes(c.v);
-    static bool attr_set = false;
-    if (!attr_set) { cudaFuncSetAttribute(k_lambda2_g, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_set = true; }
-    k_lambda2_g<<<grid, 32 * LG_WARPS, smem, st>>>(s.gpart, c.L2p, s.xr, c.o, c.v, Nc, c.npair); S_K();
-    const long long n = (long long)c.v * Nc;
-    k_g_reduce<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(s.gvec, s.gpart, s.g_blocks, n); S_K();
-    dim3 gg(nq, nret);
-    k_assemble_G<<<gg, 256, 0, st>>>(Gq, qlist, nq, s.xr, s.gvec, c.D, c.t1, c.l1, c.o, c.v, B, s.ret_row); S_K();
-    if (X1out && X2out) {
-      dim3 blk(32, 8), g2((unsigned)((c.nvec + 31) / 32), (unsigned)((nret + 31) / 32));
-      k_vec_to_abi<<<g2, blk, 0, st>>>((double2*)X1out, (double2*)X2out, s.xr, c.o, c.v, nret, B, s.ret_row); S_K();
-      const long long tot = (long long)nret * c.o * c.v;
-      k_zero_diag<<<(unsigned)std::min<long long>(4096, (tot + 255) / 256), 256, 0, st>>>((double2*)X2out, c.o, c.v, nret, s.ret_row); S_K();
-    }
+    int rc = hooks.finish(s.xr, B, nret, s.ret_row, nlaunch);
+    if (rc) { err = "G assembly failed"; return rc; }
     S_CUDA(cudaStreamSynchronize(st));   // ret_task is reused
     nret = 0; ret_task.clear();
     return 0;
@@ -595,8 +588,8 @@ struct SolveRun {
       S_CUDA(cudaMemsetAsync(s.stat + B + sl, 0, sizeof(int), st));
       S_CUDA(cudaMemsetAsync(s.stat + 2 * B + sl, 0, sizeof(int), st));
     }
-    k_build_rhs<<<nbv(nnew), 256, 0, st>>>(s.b, s.p_col, c.t1, c.T2p, c.o, c.v, A, c.nvec, c0); S_K();
-    k_x0<<<(unsigned)(c.npair + 1), 256, 0, st>>>(s.x, s.b, s.omega_col, c.eta, c.fdiag, c.o, c.v, A, c.x0, c0); S_K();
+    int rc = hooks.init(s.b, s.x, A, c0, s.p_col, s.omega_col, nlaunch);
+    if (rc) { err = "right-hand side / initial guess failed"; return rc; }
     S_TRY(dots(s.vptr + s.mcap + 2, 1, s.b, s.bn2));   // ||b||^2 of every active column (the old ones are recomputed: same value)
     return 0;
   }
@@ -715,14 +708,13 @@ struct SolveRun {
   }
 };
 
-// Solve all tasks; G rows Gq[task][iq] (device), optional X outputs in the C-ABI layout (device), statistics in `s`.
+// Solve all tasks; the hooks build the right-hand sides and consume the solutions.  Statistics in `s`.
 // Returns 0, -4 (some task not converged) or a negative error code.
-inline int solve_run(SolveWs& s, const SolveCfg& c, std::vector<SolveTask>& tasks, const SigmaFn& sigma, double2* Gq,
-                     const int* qlist, int nq, double* X1out, double* X2out, std::vector<std::vector<double>>* hist_out,
-                     double* nlaunch, std::string& err) {
+inline int solve_run(SolveWs& s, const SolveCfg& c, std::vector<SolveTask>& tasks, const SigmaFn& sigma, const SolveHooks& hooks,
+                     std::vector<std::vector<double>>* hist_out, double* nlaunch, std::string& err) {
   int rc = solve_prepare(s, c, err);
   if (rc) return rc;
-  SolveRun run{s, c, sigma, err, nlaunch, tasks, Gq, qlist, nq, X1out, X2out, hist_out, c.stream, c.batch};
+  SolveRun run{s, c, sigma, hooks, err, nlaunch, tasks, hist_out, c.stream, c.batch};
   rc = run.run();
   if (rc) return rc;
   bool conv = true;
