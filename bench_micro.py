@@ -60,8 +60,76 @@ def main():
     ap.add_argument("--ozaki-shapes", type=int, default=0)
     ap.add_argument("--slices", type=int, default=7)
     ap.add_argument("--reps", type=int, default=3)
+    ap.add_argument("--sigma-once", type=int, default=-1,
+                    help="config id: gfcc_create + ONE batched gfcc_sigma_ip on the seeded trial vectors (the short command ncu wraps "
+                         "with NVTX range filters, e.g. --nvtx --nvtx-include 'S11 Z4 = T2 V/')")
+    ap.add_argument("--mor", type=int, default=-1,
+                    help="config id: MOR step at a size that means something (SURVEY 8f rows 1, 3): two levels of converged solves at "
+                         "omega above the poles, Gram-Schmidt + projection, reduced solves on a fine grid; times per phase and the "
+                         "interpolation error against direct solves")
     a = ap.parse_args()
     out = {}
+    if a.mor >= 0:
+        import numpy as np
+        import gfcc_inputs as gi
+        c = gi.CONFIGS[a.mor]
+        s = gi.make_config(a.mor, "cuda")
+        h = g.gfcc_create(c["o"], c["v"], c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+        targets = gi.targets(a.mor)[:4]
+        wmin, wmax, dw, eta, tol = 0.40, 0.56, 0.01, c["eta"], 1e-8
+        fine = wmin + dw * np.arange(int(round((wmax - wmin) / dw)) + 1)
+        g.gfcc_set_option(h, "gmres_m", 700)
+        g.gfcc_set_option(h, "gmres_maxit", 2800)
+        g.gfcc_mor_reset(h, 2 * len(targets) * 9)
+
+        def timed(fn):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            r = fn()
+            e1.record()
+            torch.cuda.synchronize()
+            return r, e0.elapsed_time(e1)
+
+        levels = [[fine[0], fine[len(fine) // 2], fine[-1]], [fine[len(fine) // 4], fine[3 * len(fine) // 4]]]
+        rec = []
+        for lv, ws in enumerate(levels):
+            (G, X1, X2), ms_solve = timed(lambda: g.gfcc_solve_ip(h, targets, ws, eta, tol, return_x=True))
+            its = g.gfcc_get_residuals(h, len(targets) * len(ws))[1]
+            m, ms_ext = timed(lambda: g.gfcc_mor_extend(h, X1, X2, 1e-8))
+            del X1, X2
+            (Gh, A), ms_red = timed(lambda: g.gfcc_mor_solve(h, targets, fine, eta))
+            rec.append({"level": lv + 1, "omegas": [float(w) for w in ws], "m": m, "solve_ms": ms_solve, "gmres_iterations_min_max": [int(its.min()), int(its.max())],
+                        "extend_ms (Gram-Schmidt + projection)": ms_ext, "reduced_solves_ms (fine grid, %d points)" % len(fine): ms_red,
+                        "A_fine": [float(x) for x in A]})
+        # interpolation check at grid points that were NOT sampled: direct converged solves
+        chk = [fine[1], fine[len(fine) // 2 + 2]]
+        Gd = g.gfcc_solve_ip(h, targets, chk, eta, tol)
+        Ad = [float(np.trace(Gd[k]).imag / np.pi) for k in range(len(chk))]
+        idx = [1, len(fine) // 2 + 2]
+        out["mor"] = {"config": a.mor, "targets": targets, "window": [wmin, wmax, dw], "levels": rec,
+                      "check_omegas": [float(w) for w in chk], "A_direct": Ad, "A_model": [rec[-1]["A_fine"][k] for k in idx],
+                      "rel_err": [abs(rec[-1]["A_fine"][k] - Ad[q]) / abs(Ad[q]) for q, k in enumerate(idx)]}
+        g.gfcc_destroy(h)
+    if a.sigma_once >= 0:
+        import gfcc_inputs as gi
+        c = gi.CONFIGS[a.sigma_once]
+        s = gi.make_config(a.sigma_once, "cuda")
+        h = g.gfcc_create(c["o"], c["v"], c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+        del s["Lchol"]
+        torch.cuda.empty_cache()
+        nrhs = c["np"] * c["nw"] if a.sigma_once >= 2 else 64
+        X1, X2 = gi.trial_vectors(c["o"], c["v"], nrhs, gi.seed_of(a.sigma_once), "cuda")
+        w = [c["wlo"]] * nrhs
+        for _ in range(max(1, a.reps if a.reps < 3 else 1)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            g.gfcc_sigma_ip(h, w, c["eta"], X1, X2)
+            e1.record()
+            torch.cuda.synchronize()
+        out["sigma_once"] = {"config": a.sigma_once, "nrhs": nrhs, "ms": e0.elapsed_time(e1), "panel_ni": g.gfcc_get_stat(h, "panel_ni"),
+                             "tflops": g.gfcc_get_stat(h, "flops_sigma") / e0.elapsed_time(e1) / 1e9}
+        g.gfcc_destroy(h)
     if a.probe:
         out["fp64_dmma_peak_tflops"] = g.gfcc_probe_fp64_peak(20000, 5)
         x = torch.empty(1 << 28, dtype=torch.float64, device="cuda")

@@ -27,7 +27,7 @@ CONFIGS = {
 }
 
 # tensor ids
-TID_EPS_O, TID_EPS_V, TID_L, TID_T1, TID_L1, TID_T2, TID_L2, TID_X1, TID_X2 = range(1, 10)
+TID_EPS_O, TID_EPS_V, TID_L, TID_T1, TID_L1, TID_T2, TID_L2, TID_X1, TID_X2, TID_Y1, TID_Y2 = range(1, 12)
 
 _M32 = 0xFFFFFFFF
 
@@ -182,6 +182,22 @@ def trial_vectors(o, v, nrhs, seed, device="cpu"):
         X2[r, iu[0], iu[1], :] = z
         X2[r, iu[1], iu[0], :] = -z
     return X1, X2
+
+
+def trial_vectors_ea(o, v, nrhs, seed, device="cpu"):
+    """EA-type trial vectors (Eq. 4): Y1 [nrhs,v], Y2 [nrhs,o,v,v] complex128 ~ N(0,1)+iN(0,1), Y2 antisymmetrised in
+    (a,b); canonical element (r, j, a<b)."""
+    y1 = normal(seed, TID_Y1, _arange(nrhs * v * 2, device)).reshape(nrhs, v, 2)
+    Y1 = torch.complex(y1[..., 0], y1[..., 1])
+    Y2 = torch.zeros((nrhs, o, v, v), dtype=torch.complex128, device=device)
+    au = torch.triu_indices(v, v, 1, device=device)
+    T = au.shape[1]
+    for r in range(nrhs):
+        g = normal(seed, TID_Y2, _arange(o * T * 2, device, r * o * T * 2)).reshape(o, T, 2)
+        z = torch.complex(g[..., 0], g[..., 1])
+        Y2[r][:, au[0], au[1]] = z
+        Y2[r][:, au[1], au[0]] = -z
+    return Y1, Y2
 
 
 def omega_grid(cfg):

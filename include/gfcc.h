@@ -98,6 +98,9 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *                  dropped from every live vector, so the GEMM N dimension of the following sigma applications shrinks; free
  *                  columns are refilled from the pending (p,omega) list at the next restart boundary.  Default 0.125; < 0: never
  *                  (lock-step batch with a done mask; same G)
+ *   "graph"        CUDA graph of one sigma application inside gfcc_solve_ip (captured once per batch width, replayed afterwards):
+ *                  -1 (default) only for latency-bound systems (< 5 GFLOP per application), 0 never, 1 always; the statistic
+ *                  "graph_launches" counts replays and "kernel_launches" still counts every kernel a replay runs
  *   "release_workspace"  (any value) free the per-batch sigma workspace and the GMRES basis now; they are re-allocated on demand
  *   "gmres_poll"   the done flags live on the device; the host reads them every gmres_poll Arnoldi steps (0 = default: every step
  *                  when one sigma application is >= 5 GFLOP, else every 4th step)

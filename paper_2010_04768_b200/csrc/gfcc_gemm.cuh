@@ -20,6 +20,8 @@
 //   Exactly one of (sAm, sAk0) and one of (sBk0, sBn) is 1 (template flags A_KC / B_NC).
 //   C(m, n) = C + (m/Md)*sCm1 + (m%Md)*sCm0 + (n/Nd)*sCn1 + (n%Nd)*sCn0   (two-level output scatter)
 //   batch index z: A += z*bsA (tabA/sgn += z*K1), B += z*bsB, C += z*bsC.
+//   Row-block mode (Rb > 0; A m-contiguous with tabA and sgn): A(m, k1, k0) = A + tabA[(m/Rb)*tabR + k1] + (m%Rb) + k0*sAk0 and the
+//   sign sgn[(m/Rb)*tabR + k1] is applied per row (0: the rows of that block are zero-filled).
 // =====================================================================================
 #pragma once
 #include <cuda_runtime.h>
@@ -37,6 +39,9 @@ struct GemmParams {
   int batch; long long bsA, bsB, bsC; int tab_batch_stride;   // tabA/tabB/sgn advance by this per batch
   int tiles_m, tiles_n, group_m;
   int vecA, vecB;   // 1: 16-byte cp.async legal for this operand (alignment checked on the host)
+  int Rb, tabR;     // row-block mode of the A operand (Rb > 0): row m belongs to block rb = m / Rb, its local row is m % Rb, and the
+                    // K-block offset and sign are tabA[rb*tabR + k1], sgn[rb*tabR + k1] (several signed pair-packed T2 row blocks in
+                    // ONE launch: S11 as 3300-row panels instead of 660-row batches)
 };
 
 constexpr int GEMM_BN = 128;
@@ -98,6 +103,7 @@ struct GemmDesc {
   double alpha = 1.0, beta = 0.0;
   int batch = 1; long long bsA = 0, bsB = 0, bsC = 0; int tab_batch_stride = 0;
   bool tabs_even = true;   // caller's promise that every table offset is even (16-byte alignment)
+  int Rb = 0, tabR = 0;    // row-block mode of the A operand (see GemmParams)
 };
 
 // choose the m8-fragment count per warp (BM = 16*WMF, WMF in 4..8): the kernel runs one CTA per SM, so the launch takes
@@ -128,6 +134,7 @@ inline int pick_wmf(int M, long long N = 0, int batch = 1) {
 inline int gemm_bm(int M, long long N = 0, int batch = 1) { return GEMM_WGM * 8 * pick_wmf(M, N, batch); }
 
 cudaError_t launch_dgemm_ws(const GemmParams& p, bool a_kc, bool b_nc, bool sign, int wmf, cudaStream_t st);
+cudaError_t launch_dgemm_ws_rowblk(const GemmParams& p, bool b_nc, int wmf, cudaStream_t st);
 
 inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   if (d.M <= 0 || d.N <= 0 || d.K0 <= 0 || d.K1 <= 0 || d.batch <= 0) return cudaSuccess;   // empty: nothing to do
@@ -146,6 +153,8 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   p.batch = d.batch; p.bsA = d.bsA; p.bsB = d.bsB; p.bsC = d.bsC; p.tab_batch_stride = d.tab_batch_stride;
   const int wmf = pick_wmf(d.M, d.N, d.batch);
   const int bm = GEMM_WGM * 8 * wmf;
+  p.Rb = d.Rb; p.tabR = d.tabR;
+  if (d.Rb > 0 && (a_kc || !d.tabA || !d.sgn || d.batch != 1 || (d.Rb & 1))) return cudaErrorInvalidValue;
   p.tiles_m = (d.M + bm - 1) / bm;
   p.tiles_n = (d.N + GEMM_BN - 1) / GEMM_BN;
   p.group_m = 8;
@@ -155,6 +164,7 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   p.vecA = al16(d.A) && even(a_kc ? d.sAm : d.sAk0) && even(d.bsA) && (d.tabA ? d.tabs_even : even(d.sAk1));
   p.vecB = al16(d.B) && even(b_nc ? d.sBk0 : d.sBn) && even(d.bsB) && (d.tabB ? d.tabs_even : even(d.sBk1));
   const bool sign = d.sgn != nullptr;
+  if (d.Rb > 0) return launch_dgemm_ws_rowblk(p, b_nc, wmf, st);
   return launch_dgemm_ws(p, a_kc, b_nc, sign, wmf, st);
 }
 

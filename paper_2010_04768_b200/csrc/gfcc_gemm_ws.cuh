@@ -51,8 +51,9 @@ template <int WMF> struct GemmTileWS {
   static constexpr size_t SMEM_BYTES = (size_t)WS_STAGES * T::STAGE_ELEMS * sizeof(double) + 2 * WS_STAGES * sizeof(uint64_t);
 };
 
-template <int WMF, bool A_KC, bool B_NC, bool HAS_SIGN>
+template <int WMF, bool A_KC, bool B_NC, bool HAS_SIGN, bool ROWBLK = false>
 __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParams p) {
+  static_assert(!ROWBLK || (!A_KC && HAS_SIGN), "row-block mode: m-contiguous A with table and sign");
   using T = GemmTile<2, WMF>;
   constexpr int BM = T::BM, BN = GEMM_BN, BK = GEMM_BK, S = WS_STAGES;
   extern __shared__ __align__(16) double smem[];
@@ -84,10 +85,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
   const double* sgn = HAS_SIGN ? p.sgn + (long long)z * p.tab_batch_stride : nullptr;
   const int KT0 = (p.K0 + BK - 1) / BK;
   int nblocks = 0;   // number of non-skipped k1 blocks
-  if (HAS_SIGN) { for (int k1 = 0; k1 < p.K1; ++k1) nblocks += (sgn[k1] != 0.0) ? 1 : 0; }
-  else nblocks = p.K1;
+  if (HAS_SIGN && !ROWBLK) { for (int k1 = 0; k1 < p.K1; ++k1) nblocks += (sgn[k1] != 0.0) ? 1 : 0; }
+  else nblocks = p.K1;   // row-block mode: a K block is zero only for SOME rows of the tile, so none is skipped
   const int total = nblocks * KT0;
-  auto skip_zero = [&](int& k1) { if (HAS_SIGN) { while (k1 < p.K1 && sgn[k1] == 0.0) ++k1; } };
+  auto skip_zero = [&](int& k1) { if (HAS_SIGN && !ROWBLK) { while (k1 < p.K1 && sgn[k1] == 0.0) ++k1; } };
 
   if (tid >= WS_CONSUMER_THREADS) {
     // ================================ producer warpgroup ================================
@@ -99,13 +100,22 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
     const long long* tabB = p.tabB ? p.tabB + (long long)z * p.tab_batch_stride : nullptr;
     int ld_k1 = 0, ld_kt = 0;
     skip_zero(ld_k1);
+    // row-block mode: with BM/2 chunks per tile row dividing the producer thread count, a thread loads the same two rows in every tile
+    constexpr bool RB_FIXED = ROWBLK && (WS_PRODUCER_THREADS % (BM / 2) == 0);
+    int rb_fix = 0, lr_fix = 0, rb_k1 = -1;
+    long long rb_off = 0;
+    bool rb_nz = false;
+    if (RB_FIXED) {
+      const int gm = min(m0 + (ptid % (BM / 2)) * 2, p.M - 1);
+      rb_fix = gm / p.Rb; lr_fix = (m0 + (ptid % (BM / 2)) * 2) - rb_fix * p.Rb;
+    }
     int stage = 0;
     unsigned phase = 1;   // waiting on parity 1 of a fresh mbarrier returns immediately (first pass over the ring)
     for (int it = 0; it < total; ++it) {
       mbar_wait(&empty[stage], phase);
       double* As = smem + (size_t)stage * T::STAGE_ELEMS;
       double* Bs = As + T::A_ELEMS;
-      const long long offA = tabA ? tabA[ld_k1] : (long long)ld_k1 * p.sAk1;
+      const long long offA = ROWBLK ? 0 : (tabA ? tabA[ld_k1] : (long long)ld_k1 * p.sAk1);
       const long long offB = tabB ? tabB[ld_k1] : (long long)ld_k1 * p.sBk1;
       const int k0 = ld_kt * BK;
       if (A_KC) {   // As[BM][LDK], chunks along k
@@ -116,6 +126,38 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
           const int gm = m0 + row, gk = k0 + kc;
           const int nv = (gm < p.M) ? min(2, max(0, p.K0 - gk)) : 0;
           load_chunk(As + row * T::LDK + kc, Ab + offA + (long long)gm * p.sAm + gk, nv, p.vecA, p.A);
+        }
+      } else if (ROWBLK) {   // As[BK][LDA_M], chunks along m; a chunk's rows lie in ONE row block (Rb is even)
+        constexpr int CPR = BM / 2;
+        if (RB_FIXED) {        // this thread always loads the same two rows: block, local row and (per K block) offset / sign are cached
+          if (rb_k1 != ld_k1) {
+            const long long t = (long long)rb_fix * p.tabR + ld_k1;
+            rb_nz = sgn[t] != 0.0;
+            rb_off = rb_nz ? tabA[t] : 0;
+            rb_k1 = ld_k1;
+          }
+#pragma unroll
+          for (int c = ptid; c < BK * CPR; c += WS_PRODUCER_THREADS) {
+            const int kr = c / CPR, mc = (c % CPR) * 2;
+            const int gk = k0 + kr;
+            const int nv = (gk < p.K0 && rb_nz) ? min(2, max(0, p.M - (m0 + mc))) : 0;
+            load_chunk(As + kr * T::LDA_M + mc, Ab + rb_off + (long long)gk * p.sAk0 + lr_fix, nv, p.vecA, p.A);
+          }
+        } else {
+#pragma unroll
+          for (int c = ptid; c < BK * CPR; c += WS_PRODUCER_THREADS) {
+            const int kr = c / CPR, mc = (c % CPR) * 2;
+            const int gm = m0 + mc, gk = k0 + kr;
+            int nv = (gk < p.K0) ? min(2, max(0, p.M - gm)) : 0;
+            const int rb = gm / p.Rb, lr = gm - rb * p.Rb;
+            long long off = 0;
+            if (nv > 0) {
+              const long long t = (long long)rb * p.tabR + ld_k1;
+              if (sgn[t] == 0.0) nv = 0;               // zero-filled rows: this K block does not couple to the row block
+              else off = tabA[t];
+            }
+            load_chunk(As + kr * T::LDA_M + mc, Ab + off + (long long)gk * p.sAk0 + lr, nv, p.vecA, p.A);
+          }
         }
       } else {      // As[BK][LDA_M], chunks along m
         constexpr int CPR = BM / 2;
@@ -173,30 +215,49 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
   const int kl = lane & 3;
 
   double fa[2][WMF], fb[2][4];
-  auto load_frags = [&](int buf, int stage, int kk, unsigned smask) {
+  // row-block mode: the sign belongs to the ROW (block rb_f of fragment row f) and is applied to the A fragments; two masks per
+  // fragment row (current / next K block) are refreshed when the K block changes
+  int rbt[ROWBLK ? WMF : 1];
+  unsigned rm_cur[ROWBLK ? WMF : 1], rm_nxt[ROWBLK ? WMF : 1];
+  if (ROWBLK) {
+#pragma unroll
+    for (int f = 0; f < WMF; ++f) rbt[f] = min((m0 + arow + 8 * f) / p.Rb, (p.M - 1) / p.Rb) * p.tabR;
+  }
+  auto row_mask = [&](int f, int k1) -> unsigned { return (k1 < p.K1 && sgn[rbt[f] + k1] < 0.0) ? 0x80000000u : 0u; };
+  auto load_frags = [&](int buf, int stage, int kk, unsigned smask, const unsigned* rm) {
     const double* As = smem + (size_t)stage * T::STAGE_ELEMS;
     const double* Bs = As + T::A_ELEMS;
     const int k = kk * 4 + kl;
 #pragma unroll
-    for (int f = 0; f < WMF; ++f)
-      fa[buf][f] = A_KC ? As[(arow + 8 * f) * T::LDK + k] : As[k * T::LDA_M + arow + 8 * f];
+    for (int f = 0; f < WMF; ++f) {
+      const double av = A_KC ? As[(arow + 8 * f) * T::LDK + k] : As[k * T::LDA_M + arow + 8 * f];
+      fa[buf][f] = ROWBLK ? flip_sign(av, rm[f]) : av;
+    }
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
       const double bv = B_NC ? Bs[k * T::LDB_N + bcol + 8 * g] : Bs[(bcol + 8 * g) * T::LDK + k];
-      fb[buf][g] = HAS_SIGN ? flip_sign(bv, smask) : bv;
+      fb[buf][g] = (HAS_SIGN && !ROWBLK) ? flip_sign(bv, smask) : bv;
     }
   };
-  auto mask_of = [&](int k1) -> unsigned { return (HAS_SIGN && k1 < p.K1 && sgn[k1] < 0.0) ? 0x80000000u : 0u; };
+  auto mask_of = [&](int k1) -> unsigned { return (HAS_SIGN && !ROWBLK && k1 < p.K1 && sgn[k1] < 0.0) ? 0x80000000u : 0u; };
 
   int stage = 0;
   unsigned phase = 0;
   if (total > 0) {
+    if (ROWBLK) {
+#pragma unroll
+      for (int f = 0; f < WMF; ++f) rm_cur[f] = rm_nxt[f] = row_mask(f, c_k1);
+    }
     mbar_wait(&full[0], 0);
-    load_frags(0, 0, 0, mask_of(c_k1));
+    load_frags(0, 0, 0, mask_of(c_k1), rm_cur);
   }
   for (int it = 0; it < total; ++it) {
     int n_k1 = c_k1, n_kt = c_kt + 1;
     if (n_kt == KT0) { n_kt = 0; ++n_k1; skip_zero(n_k1); }
+    if (ROWBLK && n_k1 != c_k1) {
+#pragma unroll
+      for (int f = 0; f < WMF; ++f) rm_nxt[f] = row_mask(f, n_k1);
+    }
     const unsigned cur_mask = mask_of(c_k1), nxt_mask = mask_of(n_k1);
     int nstage = stage + 1;
     unsigned nphase = phase;
@@ -204,10 +265,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
 #pragma unroll
     for (int kk = 0; kk < BK / 4; ++kk) {
       const int cur = kk & 1, nxt = cur ^ 1;
-      if (kk + 1 < BK / 4) load_frags(nxt, stage, kk + 1, cur_mask);
+      if (kk + 1 < BK / 4) load_frags(nxt, stage, kk + 1, cur_mask, rm_cur);
       else if (it + 1 < total) {
         mbar_wait(&full[nstage], nphase);
-        load_frags(nxt, nstage, 0, nxt_mask);
+        load_frags(nxt, nstage, 0, nxt_mask, rm_nxt);
       }
 #pragma unroll
       for (int f = 0; f < WMF; ++f)
@@ -217,6 +278,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
     // every fragment of this stage has been consumed by an issued DMMA: hand the stage back to the producer
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[stage]);
+    if (ROWBLK && n_k1 != c_k1) {
+#pragma unroll
+      for (int f = 0; f < WMF; ++f) rm_cur[f] = rm_nxt[f];
+    }
     c_k1 = n_k1; c_kt = n_kt;
     stage = nstage; phase = nphase;
   }
@@ -290,6 +355,33 @@ inline cudaError_t launch_dgemm_ws_w(int wmf, const GemmParams& p, cudaStream_t 
     case 5: return launch_dgemm_ws_t<5, A_KC, B_NC, HAS_SIGN>(p, st);
     default: return launch_dgemm_ws_t<4, A_KC, B_NC, HAS_SIGN>(p, st);
   }
+}
+
+template <int WMF, bool B_NC>
+inline cudaError_t launch_dgemm_ws_rb_t(const GemmParams& p, cudaStream_t st) {
+  auto kern = dgemm_ws_kernel<WMF, false, B_NC, true, true>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GemmTileWS<WMF>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid((unsigned)(p.tiles_m * p.tiles_n), 1, 1);
+  kern<<<grid, WS_THREADS, GemmTileWS<WMF>::SMEM_BYTES, st>>>(p);
+  return cudaGetLastError();
+}
+template <bool B_NC>
+inline cudaError_t launch_dgemm_ws_rb_w(int wmf, const GemmParams& p, cudaStream_t st) {
+  switch (wmf) {
+    case 8: return launch_dgemm_ws_rb_t<8, B_NC>(p, st);
+    case 7: return launch_dgemm_ws_rb_t<7, B_NC>(p, st);
+    case 6: return launch_dgemm_ws_rb_t<6, B_NC>(p, st);
+    case 5: return launch_dgemm_ws_rb_t<5, B_NC>(p, st);
+    default: return launch_dgemm_ws_rb_t<4, B_NC>(p, st);
+  }
+}
+inline cudaError_t launch_dgemm_ws_rowblk(const GemmParams& p, bool b_nc, int wmf, cudaStream_t st) {
+  return b_nc ? launch_dgemm_ws_rb_w<true>(wmf, p, st) : launch_dgemm_ws_rb_w<false>(wmf, p, st);
 }
 
 inline cudaError_t launch_dgemm_ws(const GemmParams& p, bool a_kc, bool b_nc, bool sign, int wmf, cudaStream_t st) {

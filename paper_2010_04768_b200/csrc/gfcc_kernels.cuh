@@ -463,53 +463,58 @@ __global__ void __launch_bounds__(256) k_sigma2_epilogue(double* __restrict__ so
 // occupies for its whole life in the batch: element (k, r) lives at [k*ldc + slot[r]] (slot == nullptr: slot[r] = r), so
 // that dropping converged columns from the vectors (gfcc_solve.cuh) never moves the small arrays.
 // ------------------------------------------------------------------------------------
-// partial[blk][k][r] = sum over this block's rows of conj(V_k[row][r]) * w[row][r],  k in [0,nk), nk <= NK.
+// partial[blk][k][r] = sum over this block's rows of conj(V_k[row][r]) * w[row][r] for ALL k in [0,nk) in one launch: the basis is
+// walked in groups of NK vectors (NK complex accumulators per thread), w is re-read once per group (it stays in L2 for the small
+// systems where launch count matters, and costs 1/NK of the basis traffic for the large ones).
 // blockDim = (TX rhs lanes, TY row lanes); gridDim = (row blocks, ceil(nrhs/TX)); dynamic smem TX*TY double2.
 template <int NK>
 __global__ void k_multi_dot(double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
                             long long n, int nrhs, int nk) {
   extern __shared__ double2 sred[];
-  double2 acc[NK];
-#pragma unroll
-  for (int k = 0; k < NK; ++k) acc[k] = make_double2(0.0, 0.0);
   const long long rows_per_block = (n + gridDim.x - 1) / gridDim.x;
   const long long rbeg = (long long)blockIdx.x * rows_per_block;
   const long long rend = min(n, rbeg + rows_per_block);
   const int r = blockIdx.y * blockDim.x + threadIdx.x;
   const bool ok = r < nrhs;
-  if (ok) {
-    for (long long row = rbeg + threadIdx.y; row < rend; row += blockDim.y) {
-      const double2 wv = reinterpret_cast<const double2*>(w)[row * nrhs + r];
+  for (int k0 = 0; k0 < nk; k0 += NK) {
+    const int ng = min(NK, nk - k0);
+    double2 acc[NK];
 #pragma unroll
-      for (int k = 0; k < NK; ++k)
-        if (k < nk) {
-          const double2 vv = reinterpret_cast<const double2*>(Vs[k])[row * nrhs + r];
-          acc[k].x += vv.x * wv.x + vv.y * wv.y;   // conj(v) * w
-          acc[k].y += vv.x * wv.y - vv.y * wv.x;
-        }
-    }
-  }
+    for (int k = 0; k < NK; ++k) acc[k] = make_double2(0.0, 0.0);
+    if (ok) {
+      for (long long row = rbeg + threadIdx.y; row < rend; row += blockDim.y) {
+        const double2 wv = reinterpret_cast<const double2*>(w)[row * nrhs + r];
 #pragma unroll
-  for (int k = 0; k < NK; ++k) {
-    if (k < nk) {   // nk is block-uniform
-      sred[threadIdx.y * blockDim.x + threadIdx.x] = acc[k];
-      __syncthreads();
-      if (threadIdx.y == 0 && ok) {
-        double2 s = sred[threadIdx.x];
-        for (int yy = 1; yy < blockDim.y; ++yy) {
-          const double2 t = sred[yy * blockDim.x + threadIdx.x];
-          s.x += t.x;
-          s.y += t.y;
-        }
-        partial[((long long)blockIdx.x * nk + k) * nrhs + r] = s;
+        for (int k = 0; k < NK; ++k)
+          if (k < ng) {
+            const double2 vv = reinterpret_cast<const double2*>(Vs[k0 + k])[row * nrhs + r];
+            acc[k].x += vv.x * wv.x + vv.y * wv.y;   // conj(v) * w
+            acc[k].y += vv.x * wv.y - vv.y * wv.x;
+          }
       }
-      __syncthreads();
+    }
+#pragma unroll
+    for (int k = 0; k < NK; ++k) {
+      if (k < ng) {   // ng is block-uniform
+        sred[threadIdx.y * blockDim.x + threadIdx.x] = acc[k];
+        __syncthreads();
+        if (threadIdx.y == 0 && ok) {
+          double2 s = sred[threadIdx.x];
+          for (int yy = 1; yy < blockDim.y; ++yy) {
+            const double2 t = sred[yy * blockDim.x + threadIdx.x];
+            s.x += t.x;
+            s.y += t.y;
+          }
+          partial[((long long)blockIdx.x * nk + k0 + k) * nrhs + r] = s;
+        }
+        __syncthreads();
+      }
     }
   }
 }
-// h[k*ldc + slot[r]] (+)= sum_blk partial[blk][k][r]
+// h[k*ldc + slot[r]] = sum_blk partial[blk][k][r]  (+ add[k*ldc + slot[r]] if add != nullptr)
 __global__ void k_dot_finish(double2* __restrict__ h, const double2* __restrict__ partial, int nblk, int nk, int nrhs,
-                             int accumulate, const int* __restrict__ slot, int ldc) {
+                             const double2* __restrict__ add, const int* __restrict__ slot, int ldc) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= nk * nrhs) return;
   double2 s = make_double2(0.0, 0.0);
@@ -520,10 +525,11 @@ __global__ void k_dot_finish(double2* __restrict__ h, const double2* __restrict_
   }
   const int k = idx / nrhs, r = idx - k * nrhs;
   const long long out = (long long)k * ldc + (slot ? slot[r] : r);
-  if (accumulate) { s.x += h[out].x; s.y += h[out].y; }
+  if (add) { s.x += add[out].x; s.y += add[out].y; }
   h[out] = s;
 }
-// w[row][r] += sign * sum_k coef[k*ldc + slot[r]] * V_k[row][r]     (nk <= NK per launch)
+// w[row][r] += sign * sum_(k < nk) coef[k*ldc + slot[r]] * V_k[row][r]    all nk basis vectors in ONE launch: w is read and written
+// once, the sum lives in registers (NK independent basis loads in flight per thread)
 template <int NK>
 __global__ void k_multi_axpy(double* __restrict__ w, const double* const* __restrict__ Vs, const double2* __restrict__ coef,
                              long long n, int nrhs, int nk, double sign, const int* __restrict__ slot, int ldc) {
@@ -533,14 +539,19 @@ __global__ void k_multi_axpy(double* __restrict__ w, const double* const* __rest
     const int r = idx % nrhs;
     const int sl = slot ? slot[r] : r;
     double2 acc = reinterpret_cast<double2*>(w)[idx];
+    for (int k0 = 0; k0 < nk; k0 += NK) {
+      double2 vv[NK];
 #pragma unroll
-    for (int k = 0; k < NK; ++k)
-      if (k < nk) {
-        const double2 c = coef[(long long)k * ldc + sl];
-        const double2 vv = reinterpret_cast<const double2*>(Vs[k])[row * nrhs + r];
-        acc.x += sign * (c.x * vv.x - c.y * vv.y);
-        acc.y += sign * (c.x * vv.y + c.y * vv.x);
-      }
+      for (int k = 0; k < NK; ++k)
+        if (k0 + k < nk) vv[k] = reinterpret_cast<const double2*>(Vs[k0 + k])[row * nrhs + r];
+#pragma unroll
+      for (int k = 0; k < NK; ++k)
+        if (k0 + k < nk) {
+          const double2 c = coef[(long long)(k0 + k) * ldc + sl];
+          acc.x += sign * (c.x * vv[k].x - c.y * vv[k].y);
+          acc.y += sign * (c.x * vv[k].y + c.y * vv[k].x);
+        }
+    }
     reinterpret_cast<double2*>(w)[idx] = acc;
   }
 }
@@ -556,14 +567,6 @@ __global__ void k_scale_cols(double* __restrict__ out, const double* __restrict_
     x.y *= s;
     reinterpret_cast<double2*>(out)[idx] = x;
   }
-}
-// a[k*ldc + slot[r]] += b[k*ldc + slot[r]] for k < nk, r < nrhs (complex arrays)
-__global__ void k_cadd(double2* __restrict__ a, const double2* __restrict__ b, int nk, int nrhs, const int* __restrict__ slot, int ldc) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= nk * nrhs) return;
-  const int k = idx / nrhs, r = idx - k * nrhs;
-  const long long q = (long long)k * ldc + (slot ? slot[r] : r);
-  a[q].x += b[q].x; a[q].y += b[q].y;
 }
 // r = b - Ax
 __global__ void k_residual(double* __restrict__ r, const double* __restrict__ b, const double* __restrict__ ax, long long n2) {

@@ -80,7 +80,12 @@ struct gfcc_ctx {
   double st_oz_gemms = 0;
   // ---- options / stats ----
   double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3.2e9, opt_max_batch = 256, opt_overlap = 0;
-  double opt_compact = 0.125, opt_poll = 0;
+  double opt_compact = 0.125, opt_poll = 0, opt_graph = -1;
+  // ---- CUDA graphs of one sigma application for latency-bound (tiny) systems, keyed by the batch width ----
+  struct SigmaGraph { int nrhs; const double* d_omega; double eta; cudaGraphExec_t exec; size_t nodes; };
+  std::vector<SigmaGraph> graphs;
+  double *gx = nullptr, *gy = nullptr; long long g_elems = 0;
+  double st_graph_launches = 0;
   double st_iterations = 0, st_sigma_apps = 0, st_flops_sigma = 0, st_flops_create = 0, st_max_relres = 0, st_nunconv = 0;
   double st_gemm_launches = 0, st_kernel_launches = 0, st_flops_exec = 0;
   std::vector<double> last_relres;
@@ -160,7 +165,8 @@ static int gemm(gfcc_ctx* h, const GemmDesc& d) {
 static int gemm_splitk(gfcc_ctx* h, GemmDesc d, int S) {
   S = std::max(1, std::min(S, d.K1));
   const long long need = (long long)S * d.M * d.N;
-  if (S == 1 || d.batch != 1 || d.tabA || d.tabB || d.sgn || need > h->part_elems) return gemm(h, d);
+  // (a short reduction gains nothing from the split and costs two more launches: the small systems are latency-bound)
+  if (S == 1 || d.batch != 1 || d.tabA || d.tabB || d.sgn || need > h->part_elems || (long long)d.K1 * d.K0 <= 2048) return gemm(h, d);
   const int chunk = (d.K1 + S - 1) / S;
   // K1 blocks [z*chunk, min(K1,(z+1)*chunk)): launch full chunks as one batched GEMM, the ragged tail separately
   const int full = d.K1 / chunk;            // batches with exactly `chunk` blocks
@@ -199,8 +205,16 @@ static inline unsigned nblk(long long n, int t = 256, long long cap = 148LL * 32
 // ------------------------------------------------------------------------------------------
 #include "gfcc_ozaki_host.inl"
 
+static void graphs_clear(gfcc_ctx* h) {
+  for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
+  h->graphs.clear();
+  dev_free(h, h->gx, h->g_elems); dev_free(h, h->gy, h->g_elems);
+  h->gx = h->gy = nullptr; h->g_elems = 0;
+}
+
 static void free_workspace(gfcc_ctx* h) {
   const int o = h->o, v = h->v;
+  graphs_clear(h);   // the captured launches hold pointers into this workspace
   oz_free_ws(h);
   const long long Nc = 2LL * h->ws_nrhs, big = (long long)o * v * o * Nc;
   dev_free(h, h->XU, big); dev_free(h, h->Z, big); dev_free(h, h->V, big);
@@ -428,13 +442,27 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   // S11: Z[i][a][(j,c)] += sum_(n,f) t[i,n,f,a] V[(n,f)][(j,c)]   (T2 blocks through the pair table, sign per block)
   if (!oz) {
     NvtxRange nv("S11 Z4 = T2 V");
-    GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
-    d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
-    d.tabs_even = ((long long)v * v) % 2 == 0;
-    d.B = h->V; d.sBk1 = (long long)v * ld; d.sBk0 = ld; d.sBn = 1;
-    d.C = h->Z; d.sCm0 = ld; d.bsC = (long long)v * ld;
-    d.batch = o; d.beta = 1.0;
-    TRY(gemm(h, d));
+    if ((v & 1) == 0) {
+      // panels of panel_ni occupied indices i: ONE launch of ni*v rows whose K-block offsets and signs come from the pair table row
+      // of each row's i (row-block mode of the GEMM engine) -- 128-row tiles and full waves like the S9 panels
+      for (int i0 = 0; i0 < o; i0 += h->panel_ni) {
+        const int ni = std::min(h->panel_ni, o - i0);
+        GemmDesc d; d.M = ni * v; d.N = (int)ld; d.K1 = o; d.K0 = v;
+        d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab + (long long)i0 * o; d.sgn = h->blk_sgn + (long long)i0 * o;
+        d.Rb = v; d.tabR = o; d.tabs_even = true;
+        d.B = h->V; d.sBk1 = (long long)v * ld; d.sBk0 = ld; d.sBn = 1;
+        d.C = h->Z + (long long)i0 * v * ld; d.sCm0 = ld; d.beta = 1.0;
+        TRY(gemm(h, d));
+      }
+    } else {   // odd v: one batch entry per i (16-byte chunks would straddle row blocks)
+      GemmDesc d; d.M = v; d.N = (int)ld; d.K1 = o; d.K0 = v;
+      d.A = h->T2p; d.sAm = 1; d.sAk0 = v; d.tabA = h->blk_tab; d.sgn = h->blk_sgn; d.tab_batch_stride = o;
+      d.tabs_even = ((long long)v * v) % 2 == 0;
+      d.B = h->V; d.sBk1 = (long long)v * ld; d.sBk0 = ld; d.sBn = 1;
+      d.C = h->Z; d.sCm0 = ld; d.bsC = (long long)v * ld;
+      d.batch = o; d.beta = 1.0;
+      TRY(gemm(h, d));
+    }
   }
   // S13: shift + P(ij) ring
   NvtxRange nv_s13("S13 epilogue");
@@ -455,6 +483,50 @@ static double sigma_flops(const gfcc_ctx* h, int nrhs) {
   f += 2 * np_ * v * v * Nc + 2 * np_ * v * o * Nc;   // S12, S5
   f += 2 * Q * o * v * Nc + 2 * Q * o * o * Nc + 2 * ov * o * Nc;   // yv, sigma1
   return f;
+}
+
+// One sigma application through a CUDA graph (SURVEY.md section 7 "hard parts": config 0 is launch/latency-bound, ~2e8 flop per
+// application in ~20 launches).  The graph is captured once per (batch width, omega array, eta) on fixed staging vectors gx -> gy;
+// a replay costs two device copies and one graph launch on the host instead of ~20 kernel launches.
+static int sigma_via_graph(gfcc_ctx* h, int nrhs, const double* d_omega, double eta, const double* xin, double* sout) {
+  cudaStream_t st = h->stream;
+  const long long need = h->nvec * 2LL * h->ws_nrhs, elems = h->nvec * 2LL * nrhs;
+  if (h->g_elems < need) {
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    graphs_clear(h);
+    TRY(dev_alloc(h, &h->gx, need));
+    int rc = dev_alloc(h, &h->gy, need);
+    if (rc) { dev_free(h, h->gx, need); h->gx = nullptr; return rc; }
+    h->g_elems = need;
+  }
+  CUDA_TRY(h, cudaMemcpyAsync(h->gx, xin, (size_t)elems * 8, cudaMemcpyDeviceToDevice, st));
+  const gfcc_ctx::SigmaGraph* found = nullptr;
+  for (const auto& g : h->graphs) if (g.nrhs == nrhs && g.d_omega == d_omega && g.eta == eta) found = &g;
+  if (found) {
+    CUDA_TRY(h, cudaGraphLaunch(found->exec, st));
+    h->st_sigma_apps += 1; h->st_graph_launches += 1; h->st_kernel_launches += (double)found->nodes;
+  } else {
+    TRY(sigma_internal(h, nrhs, d_omega, eta, h->gx, h->gy));       // eager: a valid result, and every kernel attribute gets configured
+    const double k0 = h->st_kernel_launches, g0 = h->st_gemm_launches, f0 = h->st_flops_exec, a0 = h->st_sigma_apps;
+    cudaGraph_t graph = nullptr;
+    // the legacy default stream cannot be captured: record on a side stream then (the replay is launched on the handle's stream)
+    cudaStream_t cap = (st == nullptr || st == cudaStreamLegacy || st == cudaStreamPerThread) ? h->sB : st;
+    bool ok = cap != nullptr && cudaStreamBeginCapture(cap, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+    if (ok) {
+      h->stream = cap;
+      const int rc = sigma_internal(h, nrhs, d_omega, eta, h->gx, h->gy);
+      h->stream = st; h->cur = st;
+      ok = (cudaStreamEndCapture(cap, &graph) == cudaSuccess) && rc == GFCC_OK && graph != nullptr;
+    }
+    h->st_kernel_launches = k0; h->st_gemm_launches = g0; h->st_flops_exec = f0; h->st_sigma_apps = a0;
+    gfcc_ctx::SigmaGraph g{nrhs, d_omega, eta, nullptr, 0};
+    if (ok) ok = cudaGraphInstantiate(&g.exec, graph, 0) == cudaSuccess;
+    if (ok) { cudaGraphGetNodes(graph, nullptr, &g.nodes); h->graphs.push_back(g); }
+    else { cudaGetLastError(); h->opt_graph = 0; }                  // capture not possible here: stay on plain launches
+    if (graph) cudaGraphDestroy(graph);
+  }
+  CUDA_TRY(h, cudaMemcpyAsync(sout, h->gy, (size_t)elems * 8, cudaMemcpyDeviceToDevice, st));
+  return GFCC_OK;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -803,6 +875,7 @@ extern "C" int gfcc_destroy(gfcc_handle h) {
   if (!h) return GFCC_EINVAL;
   cudaStreamSynchronize(h->stream);
   free_side_streams(h);
+  graphs_clear(h);
   solve_free(h->sw);
   ea_destroy(h);
   for (void* p : h->allocs) cudaFree(p);
@@ -831,6 +904,7 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "max_batch" && val >= 1) h->opt_max_batch = std::floor(val);
   else if (k == "release_workspace") { cudaStreamSynchronize(h->stream); if (h->ws_nrhs) free_workspace(h); solve_free(h->sw); ea_release_ws(h); }
   else if (k == "compact" && val <= 1) h->opt_compact = val;
+  else if (k == "graph" && (val == -1 || val == 0 || val == 1)) h->opt_graph = val;
   else if (k == "gmres_poll" && val >= 0) h->opt_poll = std::floor(val);
   else if (k == "overlap" && (val == 0 || val == 1)) { h->opt_overlap = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "engine" && (val == 0 || val == 1)) { h->opt_engine = (int)val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
@@ -869,6 +943,7 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
   else if (k == "gmres_m_used") *val = h->sw.m_run;
   else if (k == "gmres_m_cap") *val = h->sw.mcap;
   else if (k == "gmres_m_memory_limit") *val = solve_mmax(h->nvec, std::max(1, h->sw.cap > 0 ? h->sw.cap : (int)h->opt_max_batch)) + (h->sw.cap > 0 ? h->sw.mcap + 6 : 0);
+  else if (k == "graph_launches") *val = h->st_graph_launches;
   else if (k == "compactions") *val = (double)h->sw.compactions;
   else if (k == "refills") *val = (double)h->sw.refills;
   else if (k == "polls") *val = (double)h->sw.polls;
@@ -894,7 +969,7 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
     }
     *val = (k == "gemm_time_ms") ? ms : (k == "gemm_flops_timed") ? fl : (k == "gemm_time_max_ms") ? mx : (double)h->ev_flops.size();
   }
-  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = 0; }
+  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = h->st_graph_launches = 0; }
   else { h->err = "gfcc_get_stat: unknown key " + k; return GFCC_EINVAL; }
   return GFCC_OK;
 }
@@ -1089,8 +1164,10 @@ extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, cons
     cfg.eta = eta; cfg.tol = tol;
     cfg.t1 = h->t1; cfg.l1 = h->l1; cfg.T2p = h->T2p; cfg.L2p = h->L2p; cfg.D = h->D; cfg.fdiag = h->fdiag;
     cfg.stream = h->stream;
+    const bool tiny = sigma_flops(h, batch) < 5e9;
     SigmaFn apply = [&](int nrhs, const double* d_omega, const double* xin, double* sout) -> int {
-      return sigma_internal(h, nrhs, d_omega, eta, xin, sout);
+      const bool graph = (h->opt_graph == 1 || (h->opt_graph < 0 && tiny)) && !h->prof && h->opt_engine == 0 && h->opt_overlap == 0;
+      return graph ? sigma_via_graph(h, nrhs, d_omega, eta, xin, sout) : sigma_internal(h, nrhs, d_omega, eta, xin, sout);
     };
     cudaStream_t st = h->stream;
     SolveHooks hooks;

@@ -3,8 +3,9 @@
 //
 // GMRES (Saad & Schultz, PAPER.md ref. 85) for a batch of right-hand sides in lockstep on the
 // RHS-fastest internal vectors vec[n][2*A] (A = active columns):
-//   Arnoldi with classical Gram-Schmidt + one re-orthogonalisation (CGS2): block dots and block axpys that read each
-//   basis vector once per pass (HBM-bound, coalesced along the RHS columns);
+//   Arnoldi with classical Gram-Schmidt + one re-orthogonalisation (CGS2): ONE block-dot launch and ONE block-axpy launch per
+//   pass over the whole basis (each basis vector read once per pass, w read/written once by the axpy; HBM-bound, coalesced
+//   along the RHS columns);
 //   per-RHS complex Givens rotations / least squares in a tiny device kernel (one thread per RHS); the done flags stay on
 //   the device and are polled every `poll` steps.
 // Load balance ("convergence ... for different (omega,p) pairs would become different and lead to severe
@@ -141,7 +142,7 @@ __global__ void k_cycle_start(const double2* __restrict__ rn2, const double2* __
 // one Arnoldi column for every active RHS: H[0..j] (CGS2 coefficients), hn2 = ||w||^2.
 // Applies the previous rotations, forms the new one, updates g, decides convergence, sets the scale of v_{j+1}.
 // R is stored with the CAPACITY stride mcap + 1 per column.
-__global__ void k_givens(int j, int mcap, int nrhs, double2* __restrict__ H, const double2* __restrict__ hn2,
+__global__ void k_givens(int j, int mcap, int nrhs, double2* __restrict__ H, const double2* __restrict__ Hcorr, const double2* __restrict__ hn2,
                          double2* __restrict__ R, double2* __restrict__ cs, double* __restrict__ sn, double2* __restrict__ g,
                          double* __restrict__ res, const double2* __restrict__ bn2, double tol, int* __restrict__ done,
                          int* __restrict__ jstop, int* __restrict__ age, double* __restrict__ hist, int histcap,
@@ -152,6 +153,10 @@ __global__ void k_givens(int j, int mcap, int nrhs, double2* __restrict__ H, con
   if (done[s]) { scale[s] = 0.0; return; }
   const long long L = ldc;
   const double hn = sqrt(fmax(hn2[s].x, 0.0));
+  for (int k = 0; k <= j; ++k) {   // CGS2: h = first-pass coefficients + re-orthogonalisation correction
+    const double2 cr = Hcorr[k * L + s];
+    H[k * L + s].x += cr.x; H[k * L + s].y += cr.y;
+  }
   for (int k = 0; k < j; ++k) {
     const double2 a = H[k * L + s], b = H[(k + 1) * L + s];
     const double2 c = cs[k * L + s];
@@ -383,6 +388,7 @@ static int solve_alloc(SolveWs& s, const SolveCfg& c, int mcap, std::string& err
   S_TRY(s_alloc(s, &s.x, vecel, err)); S_TRY(s_alloc(s, &s.b, vecel, err)); S_TRY(s_alloc(s, &s.w, vecel, err));
   S_TRY(s_alloc(s, &s.xr, vecel, err)); S_TRY(s_alloc(s, &s.spare, vecel, err));
   s.dot_blocks = (int)std::min<long long>(592, std::max<long long>(1, c.nvec / 64));
+  while (s.dot_blocks > 148 && (double)s.dot_blocks * (mcap + 1) * nr * 16.0 > 512e6) s.dot_blocks /= 2;   // bound the partial-sum buffer
   s.g_blocks = (int)std::min<long long>(296, c.npair);
   s.histcap = 8192;   // residual-history entries kept per right-hand side
   S_TRY(s_alloc(s, &s.H, (long long)(mcap + 2) * nr, err));
@@ -391,7 +397,7 @@ static int solve_alloc(SolveWs& s, const SolveCfg& c, int mcap, std::string& err
   S_TRY(s_alloc(s, &s.sn, (long long)mcap * nr, err));
   S_TRY(s_alloc(s, &s.g, (long long)(mcap + 1) * nr, err));
   S_TRY(s_alloc(s, &s.y, (long long)(mcap + 1) * nr, err));
-  S_TRY(s_alloc(s, &s.part, (long long)s.dot_blocks * 8 * nr, err));
+  S_TRY(s_alloc(s, &s.part, (long long)s.dot_blocks * (mcap + 1) * nr, err));
   S_TRY(s_alloc(s, &s.hn2, nr, err)); S_TRY(s_alloc(s, &s.bn2, nr, err));
   S_TRY(s_alloc(s, &s.scale, nr, err)); S_TRY(s_alloc(s, &s.res, nr, err));
   S_TRY(s_alloc(s, &s.hist, (long long)s.histcap * nr, err));
@@ -475,23 +481,18 @@ struct SolveRun {
     S_CUDA(cudaStreamSynchronize(st));
     return 0;
   }
-  // h[k][slot] (+)= <V_k, w>  for k in [0,nk)   (groups of 8 basis vectors per pass over w)
-  int dots(const double* const* Vs, int nk, const double* w, double2* h) {
+  // h[k][slot] = <V_k, w> (+ add[k][slot]) for k in [0,nk): one launch over the whole basis + one small reduction
+  int dots(const double* const* Vs, int nk, const double* w, double2* h, const double2* add = nullptr) {
     const int TX = A >= 32 ? 32 : (A >= 16 ? 16 : (A >= 8 ? 8 : 4));
     const int TY = 256 / TX;
     dim3 blk(TX, TY), grid(s.dot_blocks, (A + TX - 1) / TX);
-    for (int k0 = 0; k0 < nk; k0 += 8) {
-      const int n = std::min(8, nk - k0);
-      k_multi_dot<8><<<grid, blk, (size_t)TX * TY * sizeof(double2), st>>>(s.part, Vs + k0, w, c.nvec, A, n); S_K();
-      k_dot_finish<<<(n * A + 127) / 128, 128, 0, st>>>(h + (long long)k0 * B, s.part, s.dot_blocks, n, A, 0, s.slot_col, B); S_K();
-    }
+    k_multi_dot<8><<<grid, blk, (size_t)TX * TY * sizeof(double2), st>>>(s.part, Vs, w, c.nvec, A, nk); S_K();
+    k_dot_finish<<<(nk * A + 127) / 128, 128, 0, st>>>(h, s.part, s.dot_blocks, nk, A, add, s.slot_col, B); S_K();
     return 0;
   }
   int axpy(double* w, const double* const* Vs, int nk, const double2* coef, double sign) {
-    for (int k0 = 0; k0 < nk; k0 += 8) {
-      const int n = std::min(8, nk - k0);
-      k_multi_axpy<8><<<nbv(A), 256, 0, st>>>(w, Vs + k0, coef + (long long)k0 * B, c.nvec, A, n, sign, s.slot_col, B); S_K();
-    }
+    if (nk <= 0) return 0;
+    k_multi_axpy<8><<<nbv(A), 256, 0, st>>>(w, Vs, coef, c.nvec, A, nk, sign, s.slot_col, B); S_K();
     return 0;
   }
   // blocking poll of the device flags: h_stat = [done | jstop | age] by slot, h_res by slot
@@ -644,11 +645,10 @@ struct SolveRun {
         // CGS2
         S_TRY(dots(s.vptr, j + 1, s.w, s.H));
         S_TRY(axpy(s.w, s.vptr, j + 1, s.H, -1.0));
-        S_TRY(dots(s.vptr, j + 1, s.w, s.y));   // y used as scratch for the correction
+        S_TRY(dots(s.vptr, j + 1, s.w, s.y));   // y: the re-orthogonalisation correction
         S_TRY(axpy(s.w, s.vptr, j + 1, s.y, -1.0));
-        k_cadd<<<((j + 1) * A + 127) / 128, 128, 0, st>>>(s.H, s.y, j + 1, A, s.slot_col, B); S_K();
         S_TRY(dots(s.vptr + s.mcap + 1, 1, s.w, s.hn2));
-        k_givens<<<(A + 127) / 128, 128, 0, st>>>(j, s.mcap, A, s.H, s.hn2, s.R, s.cs, s.sn, s.g, s.res, s.bn2, c.tol, d_done(), d_jstop(),
+        k_givens<<<(A + 127) / 128, 128, 0, st>>>(j, s.mcap, A, s.H, s.y, s.hn2, s.R, s.cs, s.sn, s.g, s.res, s.bn2, c.tol, d_done(), d_jstop(),
                                                   d_age(), s.hist, s.histcap, s.scale, fixed ? 1 : 0, s.slot_col, B); S_K();
         if (j + 1 <= s.mcap) { k_scale_cols<<<nbv(A), 256, 0, st>>>(s.V[j + 1], s.w, s.scale, c.nvec, A, s.slot_col); S_K(); }
         if (fixed) continue;

@@ -110,3 +110,39 @@ def test_config0_ea():
     for iw in range(len(ws)):
         assert np.abs(G[iw] - Gd[iw]).max() <= TOL_G * np.abs(Gd[iw]).max()
     g.gfcc_destroy(h)
+
+
+def test_config1_ea_vs_definition_form_oracle():
+    """config 1 (o=40, v=160, Q=600) at full size against values STORED by tests/golden/make_config1_ea.py (which calls only
+    oracle/ and gfcc_inputs/): sigma_EA rows of seeded trial vectors, G^A assembly, and for q = o at omega = -0.4 the GMRES
+    residual history, the unique k-step iterate and G^A from it."""
+    import gfcc_inputs as gi
+    import paper_2010_04768_b200 as g
+    gold = np.load(os.path.join(GOLD, "config1_ea.npz"))
+    c = gi.CONFIGS[1]
+    o, v = c["o"], c["v"]
+    s = gi.make_config(1, "cpu")                  # the golden file was written from CPU-drawn inputs: same bits
+    h = g.gfcc_create(o, v, c["Q"], *[s[k].cuda() for k in ("fock", "T1", "T2p", "L1", "L2p", "Lchol")])
+    nsel = int(gold["nsel"])
+    Y1, Y2 = gi.trial_vectors_ea(o, v, nsel, gi.seed_of(1), "cpu")
+    Y1, Y2 = Y1.cuda(), Y2.cuda()
+    S1, S2 = g.gfcc_sigma_ea(h, gold["omega"], float(gold["eta"]), Y1, Y2)
+    S1h, S2h = S1.cpu().numpy(), S2.cpu().numpy()
+    e1 = np.abs(S1h[:, gold["s1rows"]].T - gold["S1s"]).max() / float(gold["scale1"])
+    e2 = np.abs(np.stack([S2h[:, j, a, b] for (j, a, b) in gold["rows"]]) - gold["S2s"]).max() / float(gold["scale2"])
+    assert e1 < TOL_SIGMA and e2 < TOL_SIGMA, (e1, e2)
+    Ga = g.gfcc_assemble_g_ea(h, Y1, Y2, gold["plist"])
+    assert np.abs(Ga - gold["GA"]).max() <= TOL_G * np.abs(gold["GA"]).max()
+    k = int(gold["kfix"])
+    g.gfcc_set_option(h, "gmres_fixed", k)
+    G, X1, X2 = g.gfcc_solve_ea(h, gold["plist"], [float(gold["om"])], float(gold["eta"]), 1e-30, return_y=True)
+    g.gfcc_set_option(h, "gmres_fixed", 0)
+    iq = list(gold["plist"]).index(int(gold["q"]))
+    hist = g.gfcc_get_residual_history(h, iq)
+    assert len(hist) == k + 1 and np.abs(hist / gold["hist"] - 1).max() < 1e-6
+    X1h, X2h = X1[iq].cpu().numpy(), X2[iq].cpu().numpy()
+    sc = max(np.abs(X1h).max(), np.abs(X2h).max())
+    assert np.abs(X1h - gold["Y1k"]).max() <= 1e-8 * sc
+    assert np.abs(np.array([X2h[j, a, b] for (j, a, b) in gold["rows"]]) - gold["Y2k"]).max() <= 1e-8 * sc
+    assert np.abs(G[0, :, iq] - gold["Gk"]).max() <= TOL_G * np.abs(gold["Gk"]).max()
+    g.gfcc_destroy(h)

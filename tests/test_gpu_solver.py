@@ -115,6 +115,24 @@ def test_fixed_steps_and_lowered_restart_length_are_honoured(small):
     g.gfcc_set_option(h, "gmres_maxit", 1000)
 
 
+def test_cuda_graph_replay_gives_the_same_bits(small):
+    """latency path (config-0-like sizes): sigma replayed from a CUDA graph inside the solver = the same kernels, same bits"""
+    s, g, orc, h = small
+    o = s["o"]
+    plist, ws = [o - 1, o + 1], [-0.4, 0.3, -0.7]
+    g.gfcc_set_option(h, "gmres_m", 300)
+    out = {}
+    for mode in (0, 1):
+        g.gfcc_set_option(h, "graph", mode)
+        g.gfcc_get_stat(h, "reset_counters")
+        G, X1, X2 = g.gfcc_solve_ip(h, plist, ws, 0.02, 1e-10, return_x=True)
+        out[mode] = (G, X2.cpu().numpy(), g.gfcc_get_stat(h, "graph_launches"), g.gfcc_get_stat(h, "sigma_applications"))
+    assert out[0][2] == 0 and out[1][2] >= out[1][3] - 8          # all but the first application per batch width are replays
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    g.gfcc_set_option(h, "graph", -1)
+    g.gfcc_set_option(h, "gmres_m", 50)
+
+
 def test_assemble_g_small(small):
     """G assembly alone (gfcc_assemble_g) against the oracle's bra vectors, occupied and virtual q"""
     s, g, orc, h = small

@@ -262,3 +262,22 @@ def test_config0_rows_and_physics(cfg0):
     # the synthetic spectrum is what SURVEY.md 8c-13 says: shifted matrices stay regular only through eta
     ev = np.linalg.eigvals(H)
     assert np.isfinite(ev).all() and ev.real.max() < 20.0
+
+
+def test_sampled_rows_equal_definition_at_config1():
+    """the row-sampled (T1-dressed, factorised) oracle -- the only sigma checker at configs 1-4 -- against the DEFINITION form
+    at o = 40, v = 160, Q = 600: definition-form values stored by tests/golden/make_config1_def.py (18 minutes of plain loops),
+    row-sampled values computed here.  An indexing slip that only shows above the tiny sizes of the other pins fails this one."""
+    import os
+    import gfcc_inputs as gi
+    gold = np.load(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config1_def.npz"))
+    c = gi.CONFIGS[1]
+    o, v = c["o"], c["v"]
+    s = gi.make_config(1, "cpu")
+    orc = oracle.Oracle(o, v, c["Q"], *[s[k].numpy() for k in ("fock", "T1", "T2p", "L1", "L2p", "Lchol")], oracle.MODE_ROWS)
+    nrhs = int(gold["nrhs"])
+    X1, X2 = gi.trial_vectors(o, v, nrhs, gi.seed_of(1), "cpu")
+    rsel = [int(r) for r in gold["rsel"]]
+    R1, R2 = orc.sigma_rows(gold["omega"][rsel], c["eta"], X1[rsel].numpy(), X2[rsel].numpy(), gold["s1rows"], gold["trip"])
+    assert np.abs(R1 - gold["S1def"]).max() < 1e-12 * np.abs(gold["S1def"]).max()
+    assert np.abs(R2 - gold["S2def"]).max() < 1e-12 * np.abs(gold["S2def"]).max()
