@@ -243,6 +243,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
 
   int stage = 0;
   unsigned phase = 0;
+  const int tail4 = (p.K0 - (KT0 - 1) * BK + 3) / 4;   // k4 steps that hold data in the last tile of a K block (1..4)
   if (total > 0) {
     if (ROWBLK) {
 #pragma unroll
@@ -262,6 +263,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
     int nstage = stage + 1;
     unsigned nphase = phase;
     if (nstage == S) { nstage = 0; nphase ^= 1u; }
+    const int nk4 = (c_kt == KT0 - 1) ? tail4 : BK / 4;
 #pragma unroll
     for (int kk = 0; kk < BK / 4; ++kk) {
       const int cur = kk & 1, nxt = cur ^ 1;
@@ -270,10 +272,12 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
         mbar_wait(&full[nstage], nphase);
         load_frags(nxt, nstage, 0, nxt_mask, rm_nxt);
       }
+      if (kk < nk4) {   // the zero-padded k4 steps of a K block's last tile are skipped (warp-uniform)
 #pragma unroll
-      for (int f = 0; f < WMF; ++f)
+        for (int f = 0; f < WMF; ++f)
 #pragma unroll
-        for (int g = 0; g < 4; ++g) dmma884(acc[f][g][0], acc[f][g][1], fa[cur][f], fb[cur][g]);
+          for (int g = 0; g < 4; ++g) dmma884(acc[f][g][0], acc[f][g][1], fa[cur][f], fb[cur][g]);
+      }
     }
     // every fragment of this stage has been consumed by an issued DMMA: hand the stage back to the producer
     __syncwarp();

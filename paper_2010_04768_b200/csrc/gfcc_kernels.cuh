@@ -343,7 +343,8 @@ __global__ void k_zero_diag(double2* __restrict__ S2, int o, int v, int nrhs, co
 
 // XU[m][e][j][c] = x2[m,j,e,c]   from the packed vector (rows o + pair*v + e), antisymmetric fill.
 // One block per (m, e): the destination row (o*Nc doubles) is contiguous; the sources are Nc-double pieces, one per j.
-// 16-byte accesses (Nc is even), four independent loads in flight per thread.
+// 16-byte accesses (Nc is even), four independent loads in flight per thread.  (A shared-memory (j, e) tile transposition that makes
+// both sides 2-4 KB runs was measured SLOWER: 4.2 against 5.1 TB/s at config 2.)
 __global__ void __launch_bounds__(256) k_unpack_xu(double* __restrict__ XU, const double* __restrict__ vec, int o, int v, int Nc) {
   const int m = blockIdx.x / v, e = blockIdx.x % v;
   const int nr = Nc >> 1;                                             // complex columns
@@ -467,8 +468,8 @@ __global__ void __launch_bounds__(256) k_sigma2_epilogue(double* __restrict__ so
 // walked in groups of NK vectors (NK complex accumulators per thread), w is re-read once per group (it stays in L2 for the small
 // systems where launch count matters, and costs 1/NK of the basis traffic for the large ones).
 // blockDim = (TX rhs lanes, TY row lanes); gridDim = (row blocks, ceil(nrhs/TX)); dynamic smem TX*TY double2.
-template <int NK>
-__global__ void k_multi_dot(double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
+template <int NK, int UR>
+__global__ void __launch_bounds__(256, 3) k_multi_dot(double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
                             long long n, int nrhs, int nk) {
   extern __shared__ double2 sred[];
   const long long rows_per_block = (n + gridDim.x - 1) / gridDim.x;
@@ -482,14 +483,27 @@ __global__ void k_multi_dot(double2* __restrict__ partial, const double* const* 
 #pragma unroll
     for (int k = 0; k < NK; ++k) acc[k] = make_double2(0.0, 0.0);
     if (ok) {
-      for (long long row = rbeg + threadIdx.y; row < rend; row += blockDim.y) {
-        const double2 wv = reinterpret_cast<const double2*>(w)[row * nrhs + r];
+      const double2* vp[NK];
 #pragma unroll
-        for (int k = 0; k < NK; ++k)
-          if (k < ng) {
-            const double2 vv = reinterpret_cast<const double2*>(Vs[k0 + k])[row * nrhs + r];
-            acc[k].x += vv.x * wv.x + vv.y * wv.y;   // conj(v) * w
-            acc[k].y += vv.x * wv.y - vv.y * wv.x;
+      for (int k = 0; k < NK; ++k) vp[k] = reinterpret_cast<const double2*>(Vs[k0 + min(k, ng - 1)]);
+      // UR rows per trip: UR * (NK + 1) independent 16-byte loads in flight per thread
+#pragma unroll 1
+      for (long long row = rbeg + threadIdx.y; row < rend; row += (long long)UR * blockDim.y) {
+        double2 wv[UR], vv[UR][NK];
+#pragma unroll
+        for (int u = 0; u < UR; ++u) {
+          const long long rw = row + (long long)u * blockDim.y;
+          const bool in = rw < rend;
+          wv[u] = in ? reinterpret_cast<const double2*>(w)[rw * nrhs + r] : make_double2(0.0, 0.0);
+#pragma unroll
+          for (int k = 0; k < NK; ++k) vv[u][k] = (in && k < ng) ? vp[k][rw * nrhs + r] : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < UR; ++u)
+#pragma unroll
+          for (int k = 0; k < NK; ++k) {
+            acc[k].x += vv[u][k].x * wv[u].x + vv[u][k].y * wv[u].y;   // conj(v) * w
+            acc[k].y += vv[u][k].x * wv[u].y - vv[u][k].y * wv[u].x;
           }
       }
     }
@@ -529,30 +543,45 @@ __global__ void k_dot_finish(double2* __restrict__ h, const double2* __restrict_
   h[out] = s;
 }
 // w[row][r] += sign * sum_(k < nk) coef[k*ldc + slot[r]] * V_k[row][r]    all nk basis vectors in ONE launch: w is read and written
-// once, the sum lives in registers (NK independent basis loads in flight per thread)
-template <int NK>
-__global__ void k_multi_axpy(double* __restrict__ w, const double* const* __restrict__ Vs, const double2* __restrict__ coef,
-                             long long n, int nrhs, int nk, double sign, const int* __restrict__ slot, int ldc) {
-  const long long total = n * nrhs;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
-    const long long row = idx / nrhs;
-    const int r = idx % nrhs;
-    const int sl = slot ? slot[r] : r;
-    double2 acc = reinterpret_cast<double2*>(w)[idx];
-    for (int k0 = 0; k0 < nk; k0 += NK) {
-      double2 vv[NK];
+// once.  blockDim = (TX rhs lanes, TY row lanes): a thread owns ONE column r (its coefficient of vector k is one load per k, not per
+// element) and UR rows at a time, whose sums live in registers; the k loop is unrolled so that 4*UR independent 16-byte basis loads
+// are in flight per thread.  gridDim = (row blocks, ceil(nrhs/TX)).
+template <int UR>
+__global__ void __launch_bounds__(256) k_multi_axpy(double* __restrict__ w, const double* const* __restrict__ Vs,
+                                                    const double2* __restrict__ coef, long long n, int nrhs, int nk, double sign,
+                                                    const int* __restrict__ slot, int ldc) {
+  const int r = blockIdx.y * blockDim.x + threadIdx.x;
+  if (r >= nrhs) return;
+  const long long sl = slot ? slot[r] : r;
+  const long long TY = blockDim.y;
+  double2* __restrict__ wp = reinterpret_cast<double2*>(w);
+  for (long long row0 = (long long)blockIdx.x * UR * TY + threadIdx.y; row0 < n; row0 += (long long)gridDim.x * UR * TY) {
+    double2 acc[UR];
 #pragma unroll
-      for (int k = 0; k < NK; ++k)
-        if (k0 + k < nk) vv[k] = reinterpret_cast<const double2*>(Vs[k0 + k])[row * nrhs + r];
-#pragma unroll
-      for (int k = 0; k < NK; ++k)
-        if (k0 + k < nk) {
-          const double2 c = coef[(long long)(k0 + k) * ldc + sl];
-          acc.x += sign * (c.x * vv[k].x - c.y * vv[k].y);
-          acc.y += sign * (c.x * vv[k].y + c.y * vv[k].x);
-        }
+    for (int u = 0; u < UR; ++u) {
+      const long long row = row0 + u * TY;
+      acc[u] = row < n ? wp[row * nrhs + r] : make_double2(0.0, 0.0);
     }
-    reinterpret_cast<double2*>(w)[idx] = acc;
+#pragma unroll 4
+    for (int k = 0; k < nk; ++k) {
+      const double2* __restrict__ vp = reinterpret_cast<const double2*>(Vs[k]);
+      double2 c = coef[(long long)k * ldc + sl];
+      c.x *= sign; c.y *= sign;
+#pragma unroll
+      for (int u = 0; u < UR; ++u) {
+        const long long row = row0 + u * TY;
+        if (row < n) {
+          const double2 vv = vp[row * nrhs + r];
+          acc[u].x += c.x * vv.x - c.y * vv.y;
+          acc[u].y += c.x * vv.y + c.y * vv.x;
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < UR; ++u) {
+      const long long row = row0 + u * TY;
+      if (row < n) wp[row * nrhs + r] = acc[u];
+    }
   }
 }
 // out[row][r] = scale[slot[r]] * in[row][r]   (real scale per rhs; scale 0 masks a converged / broken-down column)

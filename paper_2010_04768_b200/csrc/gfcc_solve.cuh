@@ -486,13 +486,18 @@ struct SolveRun {
     const int TX = A >= 32 ? 32 : (A >= 16 ? 16 : (A >= 8 ? 8 : 4));
     const int TY = 256 / TX;
     dim3 blk(TX, TY), grid(s.dot_blocks, (A + TX - 1) / TX);
-    k_multi_dot<8><<<grid, blk, (size_t)TX * TY * sizeof(double2), st>>>(s.part, Vs, w, c.nvec, A, nk); S_K();
+    if (nk <= 2) { k_multi_dot<2, 4><<<grid, blk, (size_t)TX * TY * sizeof(double2), st>>>(s.part, Vs, w, c.nvec, A, nk); S_K(); }
+    else { k_multi_dot<8, 1><<<grid, blk, (size_t)TX * TY * sizeof(double2), st>>>(s.part, Vs, w, c.nvec, A, nk); S_K(); }
     k_dot_finish<<<(nk * A + 127) / 128, 128, 0, st>>>(h, s.part, s.dot_blocks, nk, A, add, s.slot_col, B); S_K();
     return 0;
   }
   int axpy(double* w, const double* const* Vs, int nk, const double2* coef, double sign) {
     if (nk <= 0) return 0;
-    k_multi_axpy<8><<<nbv(A), 256, 0, st>>>(w, Vs, coef, c.nvec, A, nk, sign, s.slot_col, B); S_K();
+    const int TX = A >= 32 ? 32 : (A >= 16 ? 16 : (A >= 8 ? 8 : 4));
+    const int TY = 256 / TX;
+    const long long rb = (c.nvec + 4LL * TY - 1) / (4LL * TY);
+    dim3 blk(TX, TY), grid((unsigned)std::max<long long>(1, std::min<long long>(148LL * 8, rb)), (A + TX - 1) / TX);
+    k_multi_axpy<4><<<grid, blk, 0, st>>>(w, Vs, coef, c.nvec, A, nk, sign, s.slot_col, B); S_K();
     return 0;
   }
   // blocking poll of the device flags: h_stat = [done | jstop | age] by slot, h_res by slot
