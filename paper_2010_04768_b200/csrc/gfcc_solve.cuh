@@ -383,6 +383,8 @@ inline int solve_mmax(long long nvec, int cap) {
 static int solve_alloc(SolveWs& s, const SolveCfg& c, int mcap, std::string& err) {
   const long long vecel = c.nvec * 2LL * c.batch;
   const int nr = c.batch;
+  // every batch vector is its own allocation: they trade places by pointer swap when the batch is compacted
+  // (staggering their start addresses to de-correlate the low address bits was measured: slower, not faster)
   s.V.assign(mcap + 1, nullptr);
   for (int k = 0; k <= mcap; ++k) S_TRY(s_alloc(s, &s.V[k], vecel, err));
   S_TRY(s_alloc(s, &s.x, vecel, err)); S_TRY(s_alloc(s, &s.b, vecel, err)); S_TRY(s_alloc(s, &s.w, vecel, err));
