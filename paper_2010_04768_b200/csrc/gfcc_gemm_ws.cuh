@@ -272,7 +272,8 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
         mbar_wait(&full[nstage], nphase);
         load_frags(nxt, nstage, 0, nxt_mask, rm_nxt);
       }
-      if (kk < nk4) {   // the zero-padded k4 steps of a K block's last tile are skipped (warp-uniform)
+      if (!ROWBLK || kk < nk4) {   // row-block mode (short K blocks: 660 = 41.25 tiles): skip the zero-padded k4 steps of a block's
+                                   // last tile (warp-uniform); elsewhere the test costs more than the padding (measured)
 #pragma unroll
         for (int f = 0; f < WMF; ++f)
 #pragma unroll

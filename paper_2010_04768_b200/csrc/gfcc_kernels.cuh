@@ -469,7 +469,8 @@ __global__ void __launch_bounds__(256) k_sigma2_epilogue(double* __restrict__ so
 // systems where launch count matters, and costs 1/NK of the basis traffic for the large ones).
 // blockDim = (TX rhs lanes, TY row lanes); gridDim = (row blocks, ceil(nrhs/TX)); dynamic smem TX*TY double2.
 template <int NK, int UR>
-__global__ void k_multi_dot(double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
+__global__ void __launch_bounds__(256, 4) k_multi_dot(   // 4 CTAs per SM: the solver's 592-block grids are exactly one wave
+double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
                             long long n, int nrhs, int nk) {
   extern __shared__ double2 sred[];
   const long long rows_per_block = (n + gridDim.x - 1) / gridDim.x;
