@@ -60,6 +60,19 @@ typedef struct gfcc_ctx* gfcc_handle;
 int gfcc_create(int o, int v, int Q, const double* fock, const double* T1, const double* T2, const double* L1,
                 const double* L2, const double* Lchol, gfcc_handle* out);
 
+/* Closed-shell (spin-restricted) inputs (Table 2 note: the paper's production code is the closed-shell one and "only
+ * deals with the alpha electrons").  SPATIAL tensors of an RHF-based CCSD calculation, no occupied / nv virtual orbitals, Ns = no+nv:
+ *   fock [Ns][Ns], T1, L1 [no][nv], T2, L2 [no][no][nv][nv] with x[i,j,a,b] = x[j,i,b,a]  (T = sum t1 E_ai + 1/2 sum t2 E_ai E_bj,
+ *   E_pq = sum_s a+_ps a_qs; same form for Lambda), Lchol [Q][Ns][Ns].  All device pointers; NONE is borrowed.
+ * The tensors are expanded to spin orbitals ON THE DEVICE (t[is,jt,as',bt'] = d(s,s')d(t,t') t2[i,j,a,b] - d(s,t')d(t,s') t2[i,j,b,a],
+ * ...) and the handle is an ordinary spin-orbital handle with o = 2 no, v = 2 nv in the ordering occupied alpha, occupied beta,
+ * virtual alpha, virtual beta: spatial orbital p with alpha spin is spin-orbital p (p < no) or 2 no + (p - no) (p >= no).  For alpha
+ * targets gfcc_solve_ip / gfcc_solve_ea return the closed-shell G_pq; G_{p beta, q beta} = G_{p alpha, q alpha}, mixed-spin elements
+ * vanish.  This entry gives the closed-shell WORKFLOW through the spin-orbital kernels; it does not realise the flop saving of a
+ * spin-adapted formulation.                                                                              */
+int gfcc_create_closed_shell(int no, int nv, int Q, const double* fock, const double* T1, const double* T2, const double* L1,
+                             const double* L2, const double* Lchol, gfcc_handle* out);
+
 /* sigma_r = (omega[r] - i eta) X_r + Hbar X_r for r = 0..nrhs-1.
  * omega [host][nrhs];  X1,S1 complex [nrhs][o];  X2,S2 complex [nrhs][o][o][v].
  * Precondition (unchecked): X2[r][i][j][a] = -X2[r][j][i][a].  S2 is returned antisymmetric.        */

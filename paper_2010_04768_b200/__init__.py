@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libgfcc_b200.so")
 
 GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 
-EXPORTS = ["gfcc_create", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
+EXPORTS = ["gfcc_create", "gfcc_create_closed_shell", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_residual_history", "gfcc_assemble_g",
            "gfcc_get_intermediate", "gfcc_last_error",
            "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
@@ -49,6 +49,7 @@ def lib():
     vp, dp, ip = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)
     ci, cd, cll = ctypes.c_int, ctypes.c_double, ctypes.c_longlong
     L.gfcc_create.argtypes = [ci, ci, ci, vp, vp, vp, vp, vp, vp, ctypes.POINTER(vp)]
+    L.gfcc_create_closed_shell.argtypes = [ci, ci, ci, vp, vp, vp, vp, vp, vp, ctypes.POINTER(vp)]
     L.gfcc_sigma_ip.argtypes = [vp, ci, dp, cd, vp, vp, vp, vp]
     L.gfcc_sigma_ip_host.argtypes = [vp, ci, dp, cd, vp, vp, vp, vp]
     L.gfcc_solve_ip.argtypes = [vp, ci, ip, ci, dp, cd, cd, vp]
@@ -131,6 +132,26 @@ def gfcc_create(o, v, Q, fock, T1, T2, L1, L2, Lchol, stream=None):
                            _dev(Lchol, f64), ctypes.byref(out))
     _check(None, rc)
     h = Handle(out, o, v, Q, (T2, L2))
+    if stream is not None:
+        gfcc_set_stream(h, stream)
+    return h
+
+
+def gfcc_create_closed_shell(no, nv, Q, fock, T1, T2, L1, L2, Lchol, stream=None):
+    """closed-shell (spin-restricted) spatial tensors -> spin-orbital handle with o = 2 no, v = 2 nv (include/gfcc.h).
+    spin_orbital(p, alpha) = p for p < no, 2 no + (p - no) otherwise."""
+    torch = _torch()
+    f64 = torch.float64
+    Ns = no + nv
+    for t, n, name in ((fock, Ns * Ns, "fock"), (T1, no * nv, "T1"), (T2, no * no * nv * nv, "T2"), (L1, no * nv, "L1"),
+                       (L2, no * no * nv * nv, "L2"), (Lchol, Q * Ns * Ns, "Lchol")):
+        if t.numel() != n:
+            raise GfccError(GFCC_EINVAL, f"{name} has {t.numel()} elements, expected {n}")
+    out = ctypes.c_void_p()
+    rc = lib().gfcc_create_closed_shell(no, nv, Q, _dev(fock, f64), _dev(T1, f64), _dev(T2, f64), _dev(L1, f64), _dev(L2, f64),
+                                        _dev(Lchol, f64), ctypes.byref(out))
+    _check(None, rc)
+    h = Handle(out, 2 * no, 2 * nv, Q, None)
     if stream is not None:
         gfcc_set_stream(h, stream)
     return h

@@ -627,4 +627,56 @@ __global__ void k_gather_cols(double* __restrict__ dst, int ldd, int dcol0, cons
   }
 }
 
+// ------------------------------------------------------------------------------------
+// closed-shell (spin-restricted) inputs -> spin-orbital tensors (gfcc_create_closed_shell).
+// Spin-orbital ordering: occupied alpha (no), occupied beta (no), virtual alpha (nv), virtual beta (nv).
+//   f[ps,qs'] = d(s,s') f[p,q]  (same for every Cholesky vector);  t[is,as'] = d(s,s') t1[i,a]
+//   t[is,jt,as',bt'] = d(s,s') d(t,t') t2[i,j,a,b] - d(s,t') d(t,s') t2[i,j,b,a]     (same for Lambda)
+// ------------------------------------------------------------------------------------
+__device__ __forceinline__ void cs_split(int P, int no, int nv, int& spin, int& p) {   // spin-orbital -> (spin, spatial index)
+  const int o = 2 * no;
+  if (P < o) { spin = P / no; p = P - spin * no; }
+  else { const int A = P - o; spin = A / nv; p = no + (A - spin * nv); }
+}
+// dst[q][P][R] = same spin ? src[q][p][r] : 0      grid.z = number of matrices
+__global__ void k_cs_expand_matrix(double* __restrict__ dst, const double* __restrict__ src, int no, int nv) {
+  const int Ns = no + nv, N = 2 * Ns;
+  const long long total = (long long)N * N;
+  const double* s = src + (long long)blockIdx.z * Ns * Ns;
+  double* d = dst + (long long)blockIdx.z * total;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    int sp, p, sr, r;
+    cs_split((int)(idx / N), no, nv, sp, p);
+    cs_split((int)(idx % N), no, nv, sr, r);
+    d[idx] = sp == sr ? s[(long long)p * Ns + r] : 0.0;
+  }
+}
+__global__ void k_cs_expand_t1(double* __restrict__ dst, const double* __restrict__ src, int no, int nv) {
+  const int o = 2 * no, v = 2 * nv;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= o * v) return;
+  const int I = idx / v, A = idx % v;
+  const int si = I / no, sa = A / nv;
+  dst[idx] = si == sa ? src[(long long)(I - si * no) * nv + (A - sa * nv)] : 0.0;
+}
+// pair-packed [I<J][A][B] (tri == 0) or fully packed [I<J][A<B] (tri == 1) spin-orbital doubles from spatial x[i][j][a][b]
+__global__ void k_cs_expand_doubles(double* __restrict__ dst, const double* __restrict__ x, int no, int nv, int tri) {
+  const int o = 2 * no, v = 2 * nv;
+  const long long npair = (long long)o * (o - 1) / 2, per = tri ? (long long)v * (v - 1) / 2 : (long long)v * v;
+  const long long total = npair * per;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const long long pr = idx / per, ab = idx - pr * per;
+    int I, J, A, B;
+    decode_pair(pr, o, I, J);
+    if (tri) decode_pair(ab, v, A, B);
+    else { A = (int)(ab / v); B = (int)(ab % v); }
+    const int si = I / no, sj = J / no, sa = A / nv, sb = B / nv;
+    const long long i = I - si * no, j = J - sj * no, a = A - sa * nv, b = B - sb * nv;
+    double val = 0.0;
+    if (si == sa && sj == sb) val += x[((i * no + j) * nv + a) * nv + b];
+    if (si == sb && sj == sa) val -= x[((i * no + j) * nv + b) * nv + a];
+    dst[idx] = val;
+  }
+}
+
 }  // namespace gfcc

@@ -871,6 +871,57 @@ extern "C" int gfcc_create(int o, int v, int Q, const double* fock, const double
   return GFCC_OK;
 }
 
+// Closed-shell (spin-restricted) entry: the spatial tensors are expanded to spin orbitals on the device and the spin-orbital
+// intermediates are built from them (include/gfcc.h).  The expanded T2 / Lambda2 are owned by the handle.
+extern "C" int gfcc_create_closed_shell(int no, int nv, int Q, const double* fock, const double* T1, const double* T2,
+                                        const double* L1, const double* L2, const double* Lchol, gfcc_handle* out) {
+  if (out) *out = nullptr;
+  if (!out || !fock || !T1 || !T2 || !L1 || !L2 || !Lchol || no < 1 || nv < 1 || Q < 1) {
+    g_create_error = "gfcc_create_closed_shell: null pointer or invalid size (need no >= 1, nv >= 1, Q >= 1)";
+    return GFCC_EINVAL;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    g_create_error = "gfcc_create_closed_shell: no CUDA device (there is no CPU fallback)";
+    cudaGetLastError();
+    return GFCC_ECUDA;
+  }
+  const int o = 2 * no, v = 2 * nv, N = o + v;
+  gfcc_ctx* h = new gfcc_ctx();
+  h->o = o; h->v = v; h->Q = Q; h->N = N;
+  h->npair = (long long)o * (o - 1) / 2; h->ntri = (long long)v * (v - 1) / 2;
+  h->nvec = o + h->npair * v;
+  double *f_so = nullptr, *t1_so = nullptr, *l1_so = nullptr, *L_so = nullptr, *t2p = nullptr, *l2p = nullptr;
+  auto run = [&]() -> int {
+    const long long NN = (long long)N * N, ov = (long long)o * v;
+    TRY(dev_alloc(h, &t2p, h->npair * v * v)); TRY(dev_alloc(h, &l2p, h->npair * h->ntri));
+    TRY(dev_alloc(h, &f_so, NN)); TRY(dev_alloc(h, &t1_so, ov)); TRY(dev_alloc(h, &l1_so, ov)); TRY(dev_alloc(h, &L_so, (long long)Q * NN));
+    cudaStream_t st = h->stream;
+    k_cs_expand_matrix<<<dim3(nblk(NN), 1, 1), 256, 0, st>>>(f_so, fock, no, nv);
+    k_cs_expand_matrix<<<dim3(nblk(NN, 256, 4096), 1, Q), 256, 0, st>>>(L_so, Lchol, no, nv);
+    k_cs_expand_t1<<<(unsigned)((ov + 127) / 128), 128, 0, st>>>(t1_so, T1, no, nv);
+    k_cs_expand_t1<<<(unsigned)((ov + 127) / 128), 128, 0, st>>>(l1_so, L1, no, nv);
+    k_cs_expand_doubles<<<nblk(h->npair * v * v), 256, 0, st>>>(t2p, T2, no, nv, 0);
+    k_cs_expand_doubles<<<nblk(h->npair * h->ntri), 256, 0, st>>>(l2p, L2, no, nv, 1);
+    h->st_kernel_launches += 6;
+    CUDA_TRY(h, cudaGetLastError());
+    h->T2p = t2p; h->L2p = l2p;
+    TRY(create_impl(h, f_so, t1_so, l1_so, L_so));
+    dev_free(h, f_so, NN); dev_free(h, t1_so, ov); dev_free(h, l1_so, ov); dev_free(h, L_so, (long long)Q * NN);
+    return GFCC_OK;
+  };
+  const int rc = run();
+  if (rc != GFCC_OK) {
+    g_create_error = h->err;
+    free_side_streams(h);
+    for (void* p : h->allocs) cudaFree(p);
+    delete h;
+    return rc;
+  }
+  *out = h;
+  return GFCC_OK;
+}
+
 extern "C" int gfcc_destroy(gfcc_handle h) {
   if (!h) return GFCC_EINVAL;
   cudaStreamSynchronize(h->stream);
