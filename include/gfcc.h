@@ -228,6 +228,22 @@ int gfcc_destroy(gfcc_handle h);
 int gfcc_dgemm(void* cuda_stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
                const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn);
 
+/* Split-K variant of gfcc_dgemm that ALLOCATES NOTHING: for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same product and operand conventions as gfcc_dgemm; K is cut into `splits` chunks
+ * (>= 1; more parallelism for tall-skinny-K products such as the sigma1 / Fock-type reductions), each chunk's partial product goes
+ * to a scratch buffer and a second kernel reduces them into C = alpha * sum + beta * C (deterministic summation order).
+ * The scratch is a file-scope `static __device__` array inside the library of GFCC_NOALLOC_SCRATCH_DOUBLES doubles (16 MiB, held by
+ * every GPU that loads the library until the process exits): the call needs  ceil(K / ceil(K/splits)) * M * N  <= that many doubles
+ * and returns GFCC_EINVAL with a message in gfcc_last_error(NULL) otherwise (as for any other invalid argument).  It calls no
+ * cudaMalloc / cudaFree / allocating library routine; the caller passes inputs and outputs (device pointers) and a stream.
+ * EVERY call on a device shares the one array: calls whose kernels may overlap on the GPU (different streams, or graphs replayed
+ * concurrently) race on it -- serialise them.  Nothing in the array has to start at zero (every partial element that is read was
+ * written by the same call); it keeps the last call's contents.  Asynchronous with respect to the host.                      */
+#define GFCC_NOALLOC_SCRATCH_DOUBLES (1LL << 21)
+int gfcc_dgemm_splitk_noalloc(void* cuda_stream, int M, int N, int K, double alpha, const double* A, long long sAm, long long sAk,
+                              const double* B, long long sBk, long long sBn, double beta, double* C, long long sCm, long long sCn,
+                              int splits);
+
 /* FP64-accurate GEMM on the INT8 tensor pipe ("Ozaki-style FP64-accurate GEMM on the low-precision
  * tensor pipes"; the contraction is Eq. 11's pattern).  Same operand conventions as gfcc_dgemm.
  * A's rows and B's columns are scaled by powers of two and cut into `nslices` (1..8) signed 7-bit digit matrices

@@ -24,7 +24,7 @@ GFCC_OK, GFCC_EINVAL, GFCC_ENOMEM, GFCC_ECUDA, GFCC_ENOCONV = 0, -1, -2, -3, -4
 EXPORTS = ["gfcc_create", "gfcc_create_closed_shell", "gfcc_sigma_ip", "gfcc_sigma_ip_host", "gfcc_solve_ip", "gfcc_solve_ip_x", "gfcc_set_stream",
            "gfcc_set_option", "gfcc_get_stat", "gfcc_get_residuals", "gfcc_get_residual_history", "gfcc_assemble_g",
            "gfcc_get_intermediate", "gfcc_last_error",
-           "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
+           "gfcc_destroy", "gfcc_dgemm", "gfcc_dgemm_splitk_noalloc", "gfcc_dgemm_ozaki", "gfcc_probe_fp64_peak", "gfcc_mor_reset", "gfcc_mor_extend", "gfcc_mor_solve",
            "gfcc_mor_get", "gfcc_spectral_adaptive", "gfcc_sigma_ea", "gfcc_solve_ea", "gfcc_solve_ea_x", "gfcc_assemble_g_ea"]
 
 
@@ -70,6 +70,7 @@ def lib():
     L.gfcc_last_error.restype = ctypes.c_char_p
     L.gfcc_destroy.argtypes = [vp]
     L.gfcc_dgemm.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll]
+    L.gfcc_dgemm_splitk_noalloc.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll, ci]
     L.gfcc_dgemm_ozaki.argtypes = [vp, ci, ci, ci, cd, vp, cll, cll, vp, cll, cll, cd, vp, cll, cll, ci, dp, dp]
     L.gfcc_probe_fp64_peak.argtypes = [vp, ci, ci, dp]
     L.gfcc_mor_reset.argtypes = [vp, ci]
@@ -318,6 +319,26 @@ def gfcc_dgemm(A, B, C=None, alpha=1.0, beta=0.0, stream=0):
                           C.stride(0), C.stride(1))
     if rc != GFCC_OK:
         raise GfccError(rc, "gfcc_dgemm failed")
+    return C
+
+
+NOALLOC_SCRATCH_DOUBLES = 1 << 21
+
+
+def gfcc_dgemm_splitk_noalloc(A, B, C, alpha=1.0, beta=0.0, splits=8, stream=0):
+    """C = alpha * A @ B + beta * C, split-K, with the partial sums in the library's built-in static device scratch: the call allocates
+    nothing (C must be given).  Raises GfccError(GFCC_EINVAL) when parts * M * N exceeds NOALLOC_SCRATCH_DOUBLES."""
+    _torch()
+    M, K = A.shape
+    K2, N = B.shape
+    assert K == K2 and tuple(C.shape) == (M, N)
+    raw = getattr(stream, "cuda_stream", stream)
+    rc = lib().gfcc_dgemm_splitk_noalloc(ctypes.c_void_p(raw), M, N, K, float(alpha), ctypes.c_void_p(A.data_ptr()), A.stride(0),
+                                         A.stride(1), ctypes.c_void_p(B.data_ptr()), B.stride(0), B.stride(1), float(beta),
+                                         ctypes.c_void_p(C.data_ptr()), C.stride(0), C.stride(1), int(splits))
+    if rc != GFCC_OK:
+        msg = lib().gfcc_last_error(None)
+        raise GfccError(rc, msg.decode() if msg else "gfcc_dgemm_splitk_noalloc failed")
     return C
 
 

@@ -15,6 +15,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <mutex>
 #include <vector>
 #include <algorithm>
 
@@ -1168,6 +1169,86 @@ extern "C" int gfcc_dgemm_ozaki(void* stream, int M, int N, int K, double alpha,
   if (rc != GFCC_OK) cudaGetLastError();
   cleanup();
   return rc;
+}
+
+// ------------------------------------------------------------------------------------------
+// gfcc_dgemm_splitk_noalloc: split-K FP64 GEMM that allocates NOTHING (include/gfcc.h).
+// The handle-based split-K path (gemm_splitk above) keeps its partial sums in h->part, a cudaMalloc'ed buffer.  Callers that must not
+// call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it) get the same two kernels -- the DMMA
+// GEMM writing one partial product per K chunk, then k_splitk_reduce -- with the partials in this file-scope device array.  Every GPU
+// that loads the library holds the array (16 MiB) until the process exits.  In HOST code the name g_noalloc_scratch is only a stand-in
+// for the symbol, NOT a device address: the address is fetched once per device with cudaGetSymbolAddress and that pointer goes to the
+// kernels.
+// ------------------------------------------------------------------------------------------
+#define GFCC_NOALLOC_SCRATCH_DOUBLES (1LL << 21)   /* 2 097 152 doubles = 16 MiB; keep in step with include/gfcc.h */
+static __device__ __align__(256) double g_noalloc_scratch[GFCC_NOALLOC_SCRATCH_DOUBLES];
+
+static int noalloc_scratch_ptr(double** out) {
+  constexpr int MAXDEV = 64;
+  static double* ptr[MAXDEV] = {nullptr};
+  static std::mutex mtx;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAXDEV) { cudaGetLastError(); return GFCC_ECUDA; }
+  std::lock_guard<std::mutex> lock(mtx);
+  if (!ptr[dev]) {   // once per device, with that device current
+    double* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p) {
+      g_create_error = std::string("gfcc_dgemm_splitk_noalloc: cudaGetSymbolAddress failed: ") + cudaGetErrorString(e);
+      cudaGetLastError();
+      return GFCC_ECUDA;
+    }
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return GFCC_OK;
+}
+
+extern "C" int gfcc_dgemm_splitk_noalloc(void* stream, int M, int N, int K, double alpha, const double* A, long long sAm,
+                                         long long sAk, const double* B, long long sBk, long long sBn, double beta, double* C,
+                                         long long sCm, long long sCn, int splits) {
+  if (M < 1 || N < 1 || K < 1 || splits < 1 || !A || !B || !C) {
+    g_create_error = "gfcc_dgemm_splitk_noalloc: null pointer or non-positive size";
+    return GFCC_EINVAL;
+  }
+  if ((sAm != 1 && sAk != 1) || (sBk != 1 && sBn != 1)) {
+    g_create_error = "gfcc_dgemm_splitk_noalloc: one stride of A and one stride of B must be 1";
+    return GFCC_EINVAL;
+  }
+  const int S = std::min(splits, K);
+  const int chunk = (K + S - 1) / S;             // K elements per part; every part is non-empty
+  const int full = K / chunk, tail = K - full * chunk;
+  const int nparts = full + (tail > 0 ? 1 : 0);
+  const long long need = (long long)nparts * M * N;
+  if (need > GFCC_NOALLOC_SCRATCH_DOUBLES) {
+    char buf[256];
+    snprintf(buf, sizeof buf, "gfcc_dgemm_splitk_noalloc: %d parts x %d x %d = %lld doubles of partial sums exceed the built-in scratch "
+             "of %lld doubles (16 MiB): use fewer splits or gfcc_dgemm", nparts, M, N, need, (long long)GFCC_NOALLOC_SCRATCH_DOUBLES);
+    g_create_error = buf;
+    return GFCC_EINVAL;
+  }
+  double* part = nullptr;
+  const int rcp = noalloc_scratch_ptr(&part);
+  if (rcp != GFCC_OK) return rcp;
+  cudaStream_t st = (cudaStream_t)stream;
+  // part[z][m][n] = sum over chunk z of A B.  beta = 0: every element of the parts in use is overwritten, nothing has to start at zero
+  // (the array keeps the previous call's contents beyond them, which nothing reads).
+  GemmDesc g; g.M = M; g.N = N; g.K0 = chunk;
+  g.A = A; g.sAm = sAm; g.sAk0 = sAk; g.B = B; g.sBk0 = sBk; g.sBn = sBn;
+  if (sAk == 1 && sAm == 1) g.sAm = (K > 1) ? K : 1;
+  g.C = part; g.sCm0 = N; g.sCn0 = 1; g.alpha = 1.0; g.beta = 0.0;
+  g.batch = full; g.bsA = (long long)chunk * sAk; g.bsB = (long long)chunk * sBk; g.bsC = (long long)M * N;
+  if (full > 0 && launch_dgemm(g, st) != cudaSuccess) { g_create_error = "gfcc_dgemm_splitk_noalloc: GEMM launch failed"; cudaGetLastError(); return GFCC_ECUDA; }
+  if (tail > 0) {
+    GemmDesc t = g;
+    t.K0 = tail; t.batch = 1;
+    t.A = A + (long long)full * chunk * sAk; t.B = B + (long long)full * chunk * sBk; t.C = part + (long long)full * M * N;
+    if (launch_dgemm(t, st) != cudaSuccess) { g_create_error = "gfcc_dgemm_splitk_noalloc: GEMM launch failed"; cudaGetLastError(); return GFCC_ECUDA; }
+  }
+  const long long tot = (long long)M * N;
+  k_splitk_reduce<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(C, part, nparts, M, N, alpha, beta, sCm, 0, M, sCn, 0, N);
+  if (cudaGetLastError() != cudaSuccess) { g_create_error = "gfcc_dgemm_splitk_noalloc: reduction launch failed"; return GFCC_ECUDA; }
+  return GFCC_OK;
 }
 
 extern "C" int gfcc_probe_fp64_peak(void* stream, int iters, int reps, double* tflops) {
