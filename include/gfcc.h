@@ -114,6 +114,10 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *   "graph"        CUDA graph of one sigma application inside gfcc_solve_ip (captured once per batch width, replayed afterwards):
  *                  -1 (default) only for latency-bound systems (< 5 GFLOP per application), 0 never, 1 always; the statistic
  *                  "graph_launches" counts replays and "kernel_launches" still counts every kernel a replay runs
+ *   "dense"        latency path for tiny systems inside gfcc_solve_ip: the real matrix Hbar_IP (n x n, n = o + o(o-1)/2*v) is built once
+ *                  per handle by applying S1-S13 to unit vectors and a sigma application becomes ONE GEMM + a shift kernel.
+ *                  -1 (default): when n <= 2048 (33 MB); 0 never; 1 whenever n <= 8192.  gfcc_sigma_ip always runs S1-S13.
+ *                  Statistic "dense_applications" counts them.  Takes precedence over "graph".
  *   "release_workspace"  (any value) free the per-batch sigma workspace and the GMRES basis now; they are re-allocated on demand
  *   "gmres_poll"   the done flags live on the device; the host reads them every gmres_poll Arnoldi steps (0 = default: every step
  *                  when one sigma application is >= 5 GFLOP, else every 4th step)

@@ -628,6 +628,38 @@ __global__ void k_gather_cols(double* __restrict__ dst, int ldd, int dcol0, cons
 }
 
 // ------------------------------------------------------------------------------------
+// dense latency path for tiny systems (gfcc_lib.cu dense_build / dense_apply)
+// ------------------------------------------------------------------------------------
+// vec[row][c] = (row == c0 + c) ? 1 : 0      n x Nc real unit columns
+__global__ void k_unit_cols(double* __restrict__ vec, long long n, int Nc, long long c0) {
+  const long long total = n * Nc;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x)
+    vec[idx] = (idx / Nc == c0 + idx % Nc) ? 1.0 : 0.0;
+}
+// H[row][c0 + c] = src[row][c] for c < nc   (H is n x n row-major, src is n x Nc)
+__global__ void k_store_cols(double* __restrict__ H, const double* __restrict__ src, long long n, int Nc, long long c0, int nc) {
+  const long long total = n * nc;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const long long row = idx / nc;
+    const int c = (int)(idx - row * nc);
+    H[row * n + c0 + c] = src[row * Nc + c];
+  }
+}
+// s[row][r] += (omega[r] - i eta) x[row][r]     (complex columns)
+__global__ void k_dense_shift(double* __restrict__ sout, const double* __restrict__ xin, const double* __restrict__ omega, double eta,
+                              long long n, int nrhs) {
+  const long long total = n * nrhs;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+    const double w = omega[idx % nrhs];
+    const double2 x = reinterpret_cast<const double2*>(xin)[idx];
+    double2 s = reinterpret_cast<double2*>(sout)[idx];
+    s.x += w * x.x + eta * x.y;
+    s.y += w * x.y - eta * x.x;
+    reinterpret_cast<double2*>(sout)[idx] = s;
+  }
+}
+
+// ------------------------------------------------------------------------------------
 // closed-shell (spin-restricted) inputs -> spin-orbital tensors (gfcc_create_closed_shell).
 // Spin-orbital ordering: occupied alpha (no), occupied beta (no), virtual alpha (nv), virtual beta (nv).
 //   f[ps,qs'] = d(s,s') f[p,q]  (same for every Cholesky vector);  t[is,as'] = d(s,s') t1[i,a]

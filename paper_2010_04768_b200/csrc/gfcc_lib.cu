@@ -81,7 +81,10 @@ struct gfcc_ctx {
   double st_oz_gemms = 0;
   // ---- options / stats ----
   double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3.2e9, opt_max_batch = 256, opt_overlap = 0;
-  double opt_compact = 0.125, opt_poll = 0, opt_graph = -1;
+  double opt_compact = 0.125, opt_poll = 0, opt_graph = -1, opt_dense = -1;
+  // ---- dense Hbar_IP (n x n, row-major) for tiny systems: sigma inside the solver = one GEMM + a shift kernel ----
+  double* Hd = nullptr; bool hd_ready = false;
+  double st_dense_apps = 0;
   // ---- CUDA graphs of one sigma application for latency-bound (tiny) systems, keyed by the batch width ----
   struct SigmaGraph { int nrhs; const double* d_omega; double eta; cudaGraphExec_t exec; size_t nodes; };
   std::vector<SigmaGraph> graphs;
@@ -530,6 +533,66 @@ static int sigma_via_graph(gfcc_ctx* h, int nrhs, const double* d_omega, double 
   return GFCC_OK;
 }
 
+// Latency path for tiny systems (SURVEY.md section 7 "hard parts": config 0 is ~2e8 flop per application in ~20 launches).  For
+// n = o + o(o-1)/2*v <= DENSE_AUTO_MAX the real matrix Hbar_IP (n x n; 3.7 MB at config 0) is built ONCE per handle by applying the
+// S1-S13 path to unit vectors (omega = eta = 0, all 2*nb real columns of a batch used: ceil(n / (2 nb)) applications), and a sigma
+// application inside gfcc_solve_ip becomes sout = Hd * xin (one DMMA GEMM, 2 n^2 Nc flop -- FEWER than the factorised route at these
+// sizes) plus the (omega - i eta) shift: 2 launches instead of ~20.  gfcc_sigma_ip itself always runs S1-S13.  Only for sizes where
+// n^2 doubles are small; the "no o^2 v^2 intermediate" rule of BASELINE.json's configs 2-4 is about sizes where this is never used.
+constexpr long long DENSE_AUTO_MAX = 2048, DENSE_HARD_MAX = 8192;
+static bool dense_wanted(const gfcc_ctx* h) {
+  if (h->prof) return false;
+  if (h->opt_dense == 1) return h->nvec <= DENSE_HARD_MAX;
+  return h->opt_dense < 0 && h->nvec <= DENSE_AUTO_MAX;
+}
+static int dense_build(gfcc_ctx* h) {
+  if (h->hd_ready) return GFCC_OK;
+  NvtxRange nv("gfcc dense Hbar build (tiny systems)");
+  const long long n = h->nvec;
+  const int nb = (int)std::max<long long>(1, std::min<long long>(128, (n + 1) / 2));
+  TRY(ensure_workspace(h, std::max(nb, h->ws_nrhs), false));
+  const long long Nc = 2LL * nb;
+  cudaStream_t st = h->stream;
+  double *vin = nullptr, *vout = nullptr, *zero = nullptr, *Hd = nullptr;
+  int rc = GFCC_OK;
+  do {
+    if ((rc = dev_alloc(h, &Hd, n * n))) break;
+    if ((rc = dev_alloc(h, &vin, n * Nc))) break;
+    if ((rc = dev_alloc(h, &vout, n * Nc))) break;
+    if ((rc = dev_alloc(h, &zero, nb))) break;
+    if (cudaMemsetAsync(zero, 0, (size_t)nb * 8, st) != cudaSuccess) { h->err = "memset failed"; rc = GFCC_ECUDA; break; }
+    for (long long c0 = 0; c0 < n && rc == GFCC_OK; c0 += Nc) {
+      const int nc = (int)std::min<long long>(Nc, n - c0);
+      k_unit_cols<<<nblk(n * Nc), 256, 0, st>>>(vin, n, (int)Nc, c0);
+      h->st_kernel_launches += 1;
+      rc = sigma_internal(h, nb, zero, 0.0, vin, vout);      // columns are independent real vectors: Hbar is real
+      if (rc) break;
+      k_store_cols<<<nblk(n * nc), 256, 0, st>>>(Hd, vout, n, (int)Nc, c0, nc);
+      h->st_kernel_launches += 1;
+    }
+    if (rc) break;
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { h->err = "dense Hbar build failed"; rc = GFCC_ECUDA; break; }
+  } while (0);
+  cudaStreamSynchronize(st);
+  dev_free(h, vin, n * Nc); dev_free(h, vout, n * Nc); dev_free(h, zero, nb);
+  if (rc != GFCC_OK) { dev_free(h, Hd, n * n); return rc; }
+  h->Hd = Hd; h->hd_ready = true;
+  return GFCC_OK;
+}
+static int dense_apply(gfcc_ctx* h, int nrhs, const double* d_omega, double eta, const double* xin, double* sout) {
+  const long long n = h->nvec, Nc = 2LL * nrhs;
+  h->cur = h->stream;
+  GemmDesc d; d.M = (int)n; d.N = (int)Nc; d.K0 = (int)n;
+  d.A = h->Hd; d.sAm = n; d.sAk0 = 1;
+  d.B = xin; d.sBk0 = Nc; d.sBn = 1;
+  d.C = sout; d.sCm0 = Nc;
+  TRY(gemm(h, d));
+  k_dense_shift<<<nblk(n * nrhs), 256, 0, h->stream>>>(sout, xin, d_omega, eta, n, nrhs);
+  KLAUNCH(h);
+  h->st_sigma_apps += 1; h->st_dense_apps += 1;
+  return GFCC_OK;
+}
+
 // ------------------------------------------------------------------------------------------
 // gfcc_create
 // ------------------------------------------------------------------------------------------
@@ -957,6 +1020,7 @@ extern "C" int gfcc_set_option(gfcc_handle h, const char* key, double val) {
   else if (k == "release_workspace") { cudaStreamSynchronize(h->stream); if (h->ws_nrhs) free_workspace(h); solve_free(h->sw); ea_release_ws(h); }
   else if (k == "compact" && val <= 1) h->opt_compact = val;
   else if (k == "graph" && (val == -1 || val == 0 || val == 1)) h->opt_graph = val;
+  else if (k == "dense" && (val == -1 || val == 0 || val == 1)) h->opt_dense = val;
   else if (k == "gmres_poll" && val >= 0) h->opt_poll = std::floor(val);
   else if (k == "overlap" && (val == 0 || val == 1)) { h->opt_overlap = val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
   else if (k == "engine" && (val == 0 || val == 1)) { h->opt_engine = (int)val; if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); } }
@@ -996,6 +1060,7 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
   else if (k == "gmres_m_cap") *val = h->sw.mcap;
   else if (k == "gmres_m_memory_limit") *val = solve_mmax(h->nvec, std::max(1, h->sw.cap > 0 ? h->sw.cap : (int)h->opt_max_batch)) + (h->sw.cap > 0 ? h->sw.mcap + 6 : 0);
   else if (k == "graph_launches") *val = h->st_graph_launches;
+  else if (k == "dense_applications") *val = h->st_dense_apps;
   else if (k == "compactions") *val = (double)h->sw.compactions;
   else if (k == "refills") *val = (double)h->sw.refills;
   else if (k == "polls") *val = (double)h->sw.polls;
@@ -1021,7 +1086,7 @@ extern "C" int gfcc_get_stat(gfcc_handle h, const char* key, double* val) {
     }
     *val = (k == "gemm_time_ms") ? ms : (k == "gemm_flops_timed") ? fl : (k == "gemm_time_max_ms") ? mx : (double)h->ev_flops.size();
   }
-  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = h->st_graph_launches = 0; }
+  else if (k == "reset_counters") { h->ev_used = 0; h->ev_flops.clear(); h->ev_ops8.clear(); *val = 0; h->st_gemm_launches = h->st_kernel_launches = h->st_flops_exec = h->st_sigma_apps = h->st_graph_launches = h->st_dense_apps = 0; }
   else { h->err = "gfcc_get_stat: unknown key " + k; return GFCC_EINVAL; }
   return GFCC_OK;
 }
@@ -1297,7 +1362,10 @@ extern "C" int gfcc_solve_ip_x(gfcc_handle h, int np, const int* p, int nw, cons
     cfg.t1 = h->t1; cfg.l1 = h->l1; cfg.T2p = h->T2p; cfg.L2p = h->L2p; cfg.D = h->D; cfg.fdiag = h->fdiag;
     cfg.stream = h->stream;
     const bool tiny = sigma_flops(h, batch) < 5e9;
+    const bool dense = dense_wanted(h);
+    if (dense) { const int rcd = dense_build(h); if (rcd != GFCC_OK) { rc_final = rcd; break; } }
     SigmaFn apply = [&](int nrhs, const double* d_omega, const double* xin, double* sout) -> int {
+      if (dense) return dense_apply(h, nrhs, d_omega, eta, xin, sout);
       const bool graph = (h->opt_graph == 1 || (h->opt_graph < 0 && tiny)) && !h->prof && h->opt_engine == 0 && h->opt_overlap == 0;
       return graph ? sigma_via_graph(h, nrhs, d_omega, eta, xin, sout) : sigma_internal(h, nrhs, d_omega, eta, xin, sout);
     };

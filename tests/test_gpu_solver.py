@@ -121,6 +121,7 @@ def test_cuda_graph_replay_gives_the_same_bits(small):
     o = s["o"]
     plist, ws = [o - 1, o + 1], [-0.4, 0.3, -0.7]
     g.gfcc_set_option(h, "gmres_m", 300)
+    g.gfcc_set_option(h, "dense", 0)              # the dense latency path would take precedence at this size
     out = {}
     for mode in (0, 1):
         g.gfcc_set_option(h, "graph", mode)
@@ -129,6 +130,33 @@ def test_cuda_graph_replay_gives_the_same_bits(small):
         out[mode] = (G, X2.cpu().numpy(), g.gfcc_get_stat(h, "graph_launches"), g.gfcc_get_stat(h, "sigma_applications"))
     assert out[0][2] == 0 and out[1][2] >= out[1][3] - 8          # all but the first application per batch width are replays
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    g.gfcc_set_option(h, "graph", -1)
+    g.gfcc_set_option(h, "dense", -1)
+    g.gfcc_set_option(h, "gmres_m", 50)
+
+
+def test_dense_latency_path_same_G_fewer_launches(small):
+    """tiny systems: sigma inside the solver through the dense Hbar_IP built once by the S1-S13 kernels (one GEMM + shift per
+    application) -- same G as the factorised path and as the oracle's dense LU, several times fewer kernels"""
+    s, g, orc, h = small
+    o = s["o"]
+    plist, ws = [o - 1, 0, o + 1], [-0.4, 0.3, -0.7]
+    Gd = orc.G_dense(plist, ws, 0.02)
+    g.gfcc_set_option(h, "gmres_m", 300)
+    g.gfcc_set_option(h, "graph", 0)
+    out = {}
+    for mode in (0, 1):
+        g.gfcc_set_option(h, "dense", mode)
+        g.gfcc_solve_ip(h, plist, ws, 0.02, 1e-11)                 # first call of a mode may build / allocate
+        g.gfcc_get_stat(h, "reset_counters")
+        G = g.gfcc_solve_ip(h, plist, ws, 0.02, 1e-11)
+        out[mode] = (G, g.gfcc_get_stat(h, "kernel_launches"), g.gfcc_get_stat(h, "dense_applications"),
+                     g.gfcc_get_stat(h, "sigma_applications"))
+        assert relmax(G, Gd) < TOL_G
+    assert out[0][2] == 0 and out[1][2] == out[1][3] > 0
+    assert relmax(out[1][0], out[0][0]) < 1e-9
+    assert out[1][1] < 0.5 * out[0][1], (out[0][1], out[1][1])
+    g.gfcc_set_option(h, "dense", -1)
     g.gfcc_set_option(h, "graph", -1)
     g.gfcc_set_option(h, "gmres_m", 50)
 
