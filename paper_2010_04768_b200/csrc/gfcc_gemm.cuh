@@ -151,7 +151,9 @@ inline cudaError_t launch_dgemm(const GemmDesc& d, cudaStream_t st) {
   p.sCn0 = d.sCn0; p.sCn1 = d.sCn1; p.Nd = d.Nd > 0 ? d.Nd : (d.N > 0 ? d.N : 1);
   p.alpha = d.alpha; p.beta = d.beta;
   p.batch = d.batch; p.bsA = d.bsA; p.bsB = d.bsB; p.bsC = d.bsC; p.tab_batch_stride = d.tab_batch_stride;
-  const int wmf = pick_wmf(d.M, d.N, d.batch);
+  // row-block mode: only tile heights whose BM/2 chunks per tile row divide the 128 producer threads keep the producer on its fast
+  // path (a thread then loads the same two rows in every tile and caches their block's table entry): 128 or 64 rows
+  const int wmf = (d.Rb > 0) ? (d.M > 64 ? 8 : 4) : pick_wmf(d.M, d.N, d.batch);
   const int bm = GEMM_WGM * 8 * wmf;
   p.Rb = d.Rb; p.tabR = d.tabR;
   if (d.Rb > 0 && (a_kc || !d.tabA || !d.sgn || d.batch != 1 || (d.Rb & 1))) return cudaErrorInvalidValue;

@@ -245,9 +245,9 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
   unsigned phase = 0;
   const int tail4 = (p.K0 - (KT0 - 1) * BK + 3) / 4;   // k4 steps that hold data in the last tile of a K block (1..4)
   if (total > 0) {
-    if (ROWBLK) {
+    if (ROWBLK) {   // masks of the current K block and, one block AHEAD, of the next (their global loads are never waited for)
 #pragma unroll
-      for (int f = 0; f < WMF; ++f) rm_cur[f] = rm_nxt[f] = row_mask(f, c_k1);
+      for (int f = 0; f < WMF; ++f) { rm_cur[f] = row_mask(f, c_k1); rm_nxt[f] = row_mask(f, c_k1 + 1); }
     }
     mbar_wait(&full[0], 0);
     load_frags(0, 0, 0, mask_of(c_k1), rm_cur);
@@ -255,10 +255,6 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
   for (int it = 0; it < total; ++it) {
     int n_k1 = c_k1, n_kt = c_kt + 1;
     if (n_kt == KT0) { n_kt = 0; ++n_k1; skip_zero(n_k1); }
-    if (ROWBLK && n_k1 != c_k1) {
-#pragma unroll
-      for (int f = 0; f < WMF; ++f) rm_nxt[f] = row_mask(f, n_k1);
-    }
     const unsigned cur_mask = mask_of(c_k1), nxt_mask = mask_of(n_k1);
     int nstage = stage + 1;
     unsigned nphase = phase;
@@ -283,9 +279,9 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
     // every fragment of this stage has been consumed by an issued DMMA: hand the stage back to the producer
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[stage]);
-    if (ROWBLK && n_k1 != c_k1) {
+    if (ROWBLK && n_k1 != c_k1) {   // block change (no block is skipped in row-block mode: n_k1 == c_k1 + 1)
 #pragma unroll
-      for (int f = 0; f < WMF; ++f) rm_cur[f] = rm_nxt[f];
+      for (int f = 0; f < WMF; ++f) { rm_cur[f] = rm_nxt[f]; rm_nxt[f] = row_mask(f, n_k1 + 1); }
     }
     c_k1 = n_k1; c_kt = n_kt;
     stage = nstage; phase = nphase;

@@ -541,7 +541,6 @@ static int sigma_via_graph(gfcc_ctx* h, int nrhs, const double* d_omega, double 
 // n^2 doubles are small; the "no o^2 v^2 intermediate" rule of BASELINE.json's configs 2-4 is about sizes where this is never used.
 constexpr long long DENSE_AUTO_MAX = 2048, DENSE_HARD_MAX = 8192;
 static bool dense_wanted(const gfcc_ctx* h) {
-  if (h->prof) return false;
   if (h->opt_dense == 1) return h->nvec <= DENSE_HARD_MAX;
   return h->opt_dense < 0 && h->nvec <= DENSE_AUTO_MAX;
 }
