@@ -266,7 +266,9 @@ __global__ void __launch_bounds__(WS_THREADS, 1) dgemm_ws_kernel(const GemmParam
       if (kk + 1 < BK / 4) load_frags(nxt, stage, kk + 1, cur_mask, rm_cur);
       else if (it + 1 < total) {
         mbar_wait(&full[nstage], nphase);
-        load_frags(nxt, nstage, 0, nxt_mask, rm_nxt);
+        // first fragments of the next tile: its K block's row masks (rm_nxt only if that tile starts a new block; warp-uniform)
+        if (ROWBLK && n_k1 != c_k1) load_frags(nxt, nstage, 0, nxt_mask, rm_nxt);
+        else load_frags(nxt, nstage, 0, nxt_mask, rm_cur);
       }
       if (!ROWBLK || kk < nk4) {   // row-block mode (short K blocks: 660 = 41.25 tiles): skip the zero-padded k4 steps of a block's
                                    // last tile (warp-uniform); elsewhere the test costs more than the padding (measured)
