@@ -473,9 +473,9 @@ __global__ void __launch_bounds__(256, 4) k_multi_dot(   // 4 CTAs per SM: the s
 double2* __restrict__ partial, const double* const* __restrict__ Vs, const double* __restrict__ w,
                             long long n, int nrhs, int nk) {
   extern __shared__ double2 sred[];
-  const long long rows_per_block = (n + gridDim.x - 1) / gridDim.x;
-  const long long rbeg = (long long)blockIdx.x * rows_per_block;
-  const long long rend = min(n, rbeg + rows_per_block);
+  // rows are dealt to the blocks round-robin (grid-stride), so that at any moment all blocks read NEIGHBOURING rows of each vector:
+  // 1 + NK sequential DRAM streams for the whole GPU instead of (1 + NK) x gridDim.x scattered ones
+  const long long rbeg = (long long)blockIdx.x * blockDim.y, rstep = (long long)gridDim.x * blockDim.y, rend = n;
   const int r = blockIdx.y * blockDim.x + threadIdx.x;
   const bool ok = r < nrhs;
   for (int k0 = 0; k0 < nk; k0 += NK) {
@@ -484,7 +484,7 @@ double2* __restrict__ partial, const double* const* __restrict__ Vs, const doubl
 #pragma unroll
     for (int k = 0; k < NK; ++k) acc[k] = make_double2(0.0, 0.0);
     if (ok && UR == 1) {   // 1 + ng loads in flight per thread (measured best for ng > 2: 5.1 TB/s at 20 vectors)
-      for (long long row = rbeg + threadIdx.y; row < rend; row += blockDim.y) {
+      for (long long row = rbeg + threadIdx.y; row < rend; row += rstep) {
         const double2 wv = reinterpret_cast<const double2*>(w)[row * nrhs + r];
 #pragma unroll
         for (int k = 0; k < NK; ++k)
@@ -499,11 +499,11 @@ double2* __restrict__ partial, const double* const* __restrict__ Vs, const doubl
 #pragma unroll
       for (int k = 0; k < NK; ++k) vp[k] = reinterpret_cast<const double2*>(Vs[k0 + min(k, ng - 1)]);
 #pragma unroll 1
-      for (long long row = rbeg + threadIdx.y; row < rend; row += (long long)UR * blockDim.y) {
+      for (long long row = rbeg + threadIdx.y; row < rend; row += (long long)UR * rstep) {
         double2 wv[UR], vv[UR][NK];
 #pragma unroll
         for (int u = 0; u < UR; ++u) {
-          const long long rw = row + (long long)u * blockDim.y;
+          const long long rw = row + (long long)u * rstep;
           const bool in = rw < rend;
           wv[u] = in ? reinterpret_cast<const double2*>(w)[rw * nrhs + r] : make_double2(0.0, 0.0);
 #pragma unroll

@@ -485,7 +485,7 @@ struct SolveRun {
   }
   // h[k][slot] = <V_k, w> (+ add[k][slot]) for k in [0,nk): one launch over the whole basis + one small reduction
   int dots(const double* const* Vs, int nk, const double* w, double2* h, const double2* add = nullptr) {
-    const int TX = A >= 32 ? 32 : (A >= 16 ? 16 : (A >= 8 ? 8 : 4));
+    const int TX = A >= 64 ? 64 : A >= 32 ? 32 : (A >= 16 ? 16 : (A >= 8 ? 8 : 4));
     const int TY = 256 / TX;
     dim3 blk(TX, TY), grid(s.dot_blocks, (A + TX - 1) / TX);
     if (nk <= 2) { k_multi_dot<2, 4><<<grid, blk, (size_t)TX * TY * sizeof(double2), st>>>(s.part, Vs, w, c.nvec, A, nk); S_K(); }
