@@ -67,8 +67,39 @@ def main():
                     help="config id: MOR step at a size that means something (SURVEY 8f rows 1, 3): two levels of converged solves at "
                          "omega above the poles, Gram-Schmidt + projection, reduced solves on a fine grid; times per phase and the "
                          "interpolation error against direct solves")
+    ap.add_argument("--adaptive", type=int, default=-1,
+                    help="config id: gfcc_spectral_adaptive (Alg. 1 level loop) over a window above the poles; wall time, levels, m, "
+                         "and A at the sampled points against direct converged solves")
     a = ap.parse_args()
     out = {}
+    if a.adaptive >= 0:
+        import time
+        import numpy as np
+        import gfcc_inputs as gi
+        c = gi.CONFIGS[a.adaptive]
+        s = gi.make_config(a.adaptive, "cuda")
+        h = g.gfcc_create(c["o"], c["v"], c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+        targets = gi.targets(a.adaptive)[:4]
+        wmin, wmax, dw, eta, tol = 0.40, 0.56, 0.01, c["eta"], 1e-8
+        g.gfcc_set_option(h, "gmres_m", 700)
+        g.gfcc_set_option(h, "gmres_maxit", 2800)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r = g.gfcc_spectral_adaptive(h, targets, wmin, wmax, dw, eta, tol, spec_tol=1e-3, droptol=1e-8)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        lev = r["level_of"]
+        sampled = [int(k) for k in np.nonzero(lev)[0]]
+        chk = [sampled[1], sampled[len(sampled) // 2]]
+        Gd = g.gfcc_solve_ip(h, targets, [float(r["w"][k]) for k in chk], eta, tol)
+        Ad = [float(np.trace(Gd[q]).imag / np.pi) for q in range(len(chk))]
+        out["adaptive"] = {"config": a.adaptive, "targets": targets, "window": [wmin, wmax, dw], "levels": int(r["levels"]), "m": int(r["m"]),
+                           "points_per_level": [int((lev == L).sum()) for L in range(1, int(r["levels"]) + 1)], "wall_s": wall,
+                           "sampled_omega": [float(r["w"][k]) for k in sampled], "check_omega": [float(r["w"][k]) for k in chk],
+                           "A_model": [float(r["A"][k]) for k in chk], "A_direct": Ad,
+                           "rel_err": [abs(float(r["A"][k]) - Ad[q]) / abs(Ad[q]) for q, k in enumerate(chk)],
+                           "A_fine": [float(x) for x in r["A"]]}
+        g.gfcc_destroy(h)
     if a.mor >= 0:
         import numpy as np
         import gfcc_inputs as gi
