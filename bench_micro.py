@@ -70,8 +70,37 @@ def main():
     ap.add_argument("--adaptive", type=int, default=-1,
                     help="config id: gfcc_spectral_adaptive (Alg. 1 level loop) over a window above the poles; wall time, levels, m, "
                          "and A at the sampled points against direct converged solves")
+    ap.add_argument("--ea-once", type=int, default=-1,
+                    help="config id (0 or 1): gfcc_create + EA preparation + timed batched gfcc_sigma_ea applications on seeded trial vectors")
     a = ap.parse_args()
     out = {}
+    if a.ea_once >= 0:
+        import gfcc_inputs as gi
+        c = gi.CONFIGS[a.ea_once]
+        s = gi.make_config(a.ea_once, "cuda")
+        h = g.gfcc_create(c["o"], c["v"], c["Q"], s["fock"], s["T1"], s["T2p"], s["L1"], s["L2p"], s["Lchol"])
+        nrhs = 32
+        Y1, Y2 = gi.trial_vectors_ea(c["o"], c["v"], nrhs, gi.seed_of(a.ea_once), "cuda")
+        w = [0.3] * nrhs
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.gfcc_sigma_ea(h, w, c["eta"], Y1, Y2)          # first call: builds W_abej and the workspace
+        e1.record()
+        torch.cuda.synchronize()
+        first_ms = e0.elapsed_time(e1)
+        best, fl = 1e30, 0.0
+        for _ in range(max(1, a.reps)):
+            f0 = g.gfcc_get_stat(h, "flops_executed")
+            e0.record()
+            g.gfcc_sigma_ea(h, w, c["eta"], Y1, Y2)
+            e1.record()
+            torch.cuda.synchronize()
+            fl = g.gfcc_get_stat(h, "flops_executed") - f0
+            best = min(best, e0.elapsed_time(e1))
+        out["ea_once"] = {"config": a.ea_once, "nrhs": nrhs, "first_call_ms (incl. W_abej build)": first_ms, "ms": best,
+                          "executed_gemm_flops": fl, "tflops_executed": fl / best / 1e9}
+        g.gfcc_destroy(h)
     if a.adaptive >= 0:
         import time
         import numpy as np
