@@ -161,7 +161,7 @@ def cpu_baseline(cfg, c, nrhs, flops_sigma, ready_cb=None):
     right-hand sides to first order: the row-sampled routine rebuilds O(o^2 v Q) intermediates per row, which is what makes it a
     checker and not a sigma implementation -- the number is a baseline, not a target)."""
     nrhs_s = 2
-    ns_small, ns_large = (2, 10) if cfg <= 2 else ((1, 5) if cfg == 3 else (1, 3))
+    ns_small, ns_large = (2, 10) if cfg <= 2 else ((1, 4) if cfg == 3 else (1, 2))   # ~65 s per sigma2 row at config 4
     t_setup, (t_a, t_b), cores = oracle_sample(cfg, c, nrhs_s, ns_small, ns_large, ready_cb)
     t_row = max((t_b - t_a) / (ns_large - ns_small), 1e-9)
     t_call = max(t_a - ns_small * t_row, 0.0)
