@@ -179,3 +179,40 @@ def test_config0_solve(cfg0):
         # 25 Arnoldi steps + 1 residual evaluation = 26 sigma applications in the oracle's counting
         x1, x2, nit, rr = orc.gmres(s["targets"][0], ws[iw], s["eta"], 1e-30, m=25, maxit=26, x0kind=1)
         assert relmax(orc.pack(X1[iw].cpu().numpy(), X2[iw].cpu().numpy()), orc.pack(x1, x2)) < 1e-8
+
+
+def test_failed_workspace_allocation_leaves_the_handle_usable():
+    """a workspace allocation that fails half-way (device memory nearly full) must return GFCC_ENOMEM and leave the
+    handle clean, so that the same call succeeds once memory is available again (no launch on half-allocated buffers)."""
+    import gc
+    s = random_system(12, 37, 50, seed=3, l_scale=0.1)
+    g, orc, h = make_pair(s)
+    o, v = 12, 37
+    x1, x2 = random_x(o, v, 4, seed=11)
+    w4 = np.array([-0.3, -0.5, 0.2, -0.9])
+    ref1, ref2 = g.gfcc_sigma_ip(h, w4, 0.01, dev(x1), dev(x2))            # loads the kernels, small workspace
+    torch.cuda.synchronize()
+    nrhs = 2048                                                            # workspace of this batch: 3 x 175 MB + vectors
+    X1 = dev(np.tile(x1, (nrhs // 4, 1)))
+    X2 = dev(np.tile(x2, (nrhs // 4, 1, 1, 1)))
+    S1 = torch.empty_like(X1)
+    S2 = torch.empty_like(X2)
+    wbig = np.tile(w4, nrhs // 4)
+    gc.collect()
+    torch.cuda.empty_cache()
+    free = torch.cuda.mem_get_info()[0]
+    hog = torch.empty(free - 300 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # leave ~300 MB: the 2nd/3rd buffer cannot fit
+    with pytest.raises(g.GfccError) as e:
+        g.gfcc_sigma_ip(h, wbig, 0.01, X1, X2, S1, S2)
+    assert e.value.code == g.GFCC_ENOMEM
+    with pytest.raises(g.GfccError) as e:                                   # again, same batch width: still an error, not a crash
+        g.gfcc_sigma_ip(h, wbig, 0.01, X1, X2, S1, S2)
+    assert e.value.code == g.GFCC_ENOMEM
+    del hog
+    torch.cuda.empty_cache()
+    g.gfcc_sigma_ip(h, wbig, 0.01, X1, X2, S1, S2)                          # memory is back: the same call works
+    torch.cuda.synchronize()
+    assert relmax(S1[:4].cpu().numpy(), ref1.cpu().numpy()) < 1e-13 and relmax(S2[-4:].cpu().numpy(), ref2.cpu().numpy()) < 1e-13
+    G1, G2 = g.gfcc_sigma_ip(h, w4, 0.01, dev(x1), dev(x2))                 # and the small batch still does
+    assert relmax(G2.cpu().numpy(), ref2.cpu().numpy()) < 1e-13
+    g.gfcc_destroy(h)
