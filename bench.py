@@ -506,7 +506,10 @@ def main():
             nb = X1h.numel() * 16 + X2h.numel() * 16
             line["e2e"] = {"value": flops_sigma / dt / 1e12, "unit": "TFLOP/s", "h2d_bytes_per_step": int(nb + 8 * nrhs),
                            "d2h_bytes_per_step": int(nb), "ms_per_step": dt * 1e3,
-                           "what": "gfcc_sigma_ip_host: X1,X2 from pinned host memory, S1,S2 back to pinned host memory, copies inside the timed call"}
+                           "what": "gfcc_sigma_ip_host: X1,X2 from pinned host memory, S1,S2 back to pinned host memory, copies inside the timed call",
+                           "note": "the timed STEP itself (gfcc_solve_ip) already takes host arrays p[], omega[] and returns G on the host; its only "
+                                   "device-resident input is the handle built by gfcc_create, so `value` is end to end for the solve step and this "
+                                   "entry adds the sigma call whose vectors (5.5 GB each way at config 4) cross PCIe"}
         except Exception as ex:   # noqa: BLE001
             line["e2e"] = {"value": None, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": str(ex)[:200]}
     # ---- extra (not the headline): the same step on the INT8 tensor-core engine, 1 warm-up + 1 timed step ----
