@@ -342,34 +342,44 @@ __global__ void k_zero_diag(double2* __restrict__ S2, int o, int v, int nrhs, co
 }
 
 // XU[m][e][j][c] = x2[m,j,e,c]   from the packed vector (rows o + pair*v + e), antisymmetric fill.
-// One block per (m, e): the destination row (o*Nc doubles) is contiguous; the sources are Nc-double pieces, one per j.
-// 16-byte accesses (Nc is even), four independent loads in flight per thread.  (A shared-memory (j, e) tile transposition that makes
-// both sides 2-4 KB runs was measured SLOWER: 4.2 against 5.1 TB/s at config 2.)
+// One block per pair (m<j): its v*Nc source doubles are contiguous and are read ONCE; both images XU[m][e][j][:] = +x and
+// XU[j][e][m][:] = -x are written from registers (Nc-double pieces).  The earlier form (one block per destination row) read every x2
+// element twice from DRAM -- once for (m,j), once for (j,m), in blocks far apart: ncu showed 2.04 GB read for 1.04 GB of x2 at config 2
+// with the DRAM pipe saturated (6.6 TB/s of real traffic).  Blocks npair .. npair+o-1 zero the diagonal XU[m][e][m][:].
 __global__ void __launch_bounds__(256) k_unpack_xu(double* __restrict__ XU, const double* __restrict__ vec, int o, int v, int Nc) {
-  const int m = blockIdx.x / v, e = blockIdx.x % v;
   const int nr = Nc >> 1;                                             // complex columns
-  double2* __restrict__ dst = reinterpret_cast<double2*>(XU + (long long)blockIdx.x * o * Nc);
-  const double2* __restrict__ x2 = reinterpret_cast<const double2*>(vec + (long long)o * Nc);
-  const int total = o * nr;
+  const long long npair = (long long)o * (o - 1) / 2;
+  double2* __restrict__ xu = reinterpret_cast<double2*>(XU);
+  const int total = v * nr;
+  if (blockIdx.x >= npair) {
+    const long long m = blockIdx.x - npair;
+    for (int t = threadIdx.x; t < total; t += blockDim.x) {
+      const int e = t / nr, c = t - e * nr;
+      xu[((m * v + e) * o + m) * nr + c] = make_double2(0.0, 0.0);
+    }
+    return;
+  }
+  int m, j;
+  decode_pair(blockIdx.x, o, m, j);
+  const double2* __restrict__ src = reinterpret_cast<const double2*>(vec + (long long)o * Nc) + (long long)blockIdx.x * total;
+  double2* __restrict__ dmj = xu + ((long long)m * v * o + j) * nr;    // + e*o*nr + c
+  double2* __restrict__ djm = xu + ((long long)j * v * o + m) * nr;
+  const long long se = (long long)o * nr;
   for (int t0 = threadIdx.x; t0 < total; t0 += 4 * blockDim.x) {
     double2 val[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int t = t0 + u * blockDim.x;
-      val[u] = make_double2(0.0, 0.0);
-      if (t < total) {
-        const int j = t / nr, c = t - j * nr;
-        if (m < j) val[u] = x2[(pair_index(m, j, o) * v + e) * nr + c];
-        else if (m > j) {
-          const double2 q = x2[(pair_index(j, m, o) * v + e) * nr + c];
-          val[u] = make_double2(-q.x, -q.y);
-        }
-      }
+      if (t < total) val[u] = src[t];
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const int t = t0 + u * blockDim.x;
-      if (t < total) dst[t] = val[u];
+      if (t < total) {
+        const int e = t / nr, c = t - e * nr;
+        dmj[e * se + c] = val[u];
+        djm[e * se + c] = make_double2(-val[u].x, -val[u].y);
+      }
     }
   }
 }

@@ -310,7 +310,7 @@ static int sigma_internal(gfcc_ctx* h, int nrhs, const double* d_omega, double e
   NvtxRange nv_sigma("gfcc sigma (S1-S13)");
   h->cur = s0;
   // XU[m][e][j][c] = x2[m,j,e]
-  k_unpack_xu<<<(unsigned)ov, 256, 0, s0>>>(h->XU, xin, o, v, (int)Nc);
+  k_unpack_xu<<<(unsigned)(h->npair + o), 256, 0, s0>>>(h->XU, xin, o, v, (int)Nc);
   KLAUNCH(h);
   // S1: Y[Q][(j,c)] = sum_(m,e) Lov[Q][(m,e)] XU[(m,e)][(j,c)]
   {
