@@ -493,13 +493,16 @@ double2* __restrict__ partial, const double* const* __restrict__ Vs, const doubl
     double2 acc[NK];
 #pragma unroll
     for (int k = 0; k < NK; ++k) acc[k] = make_double2(0.0, 0.0);
-    if (ok && UR == 1) {   // 1 + ng loads in flight per thread (measured best for ng > 2: 5.1 TB/s at 20 vectors)
+    if (ok && UR == 1) {   // 1 + ng loads in flight per thread (measured best for ng > 2: 6.0 TB/s at 20 vectors)
+      const double2* vq[NK];   // basis pointers read once per group, not once per row (no pointer -> data dependent load in the loop)
+#pragma unroll
+      for (int k = 0; k < NK; ++k) vq[k] = reinterpret_cast<const double2*>(Vs[k0 + min(k, ng - 1)]);
       for (long long row = rbeg + threadIdx.y; row < rend; row += rstep) {
         const double2 wv = reinterpret_cast<const double2*>(w)[row * nrhs + r];
 #pragma unroll
         for (int k = 0; k < NK; ++k)
           if (k < ng) {
-            const double2 vv = reinterpret_cast<const double2*>(Vs[k0 + k])[row * nrhs + r];
+            const double2 vv = vq[k][row * nrhs + r];
             acc[k].x += vv.x * wv.x + vv.y * wv.y;   // conj(v) * w
             acc[k].y += vv.x * wv.y - vv.y * wv.x;
           }
