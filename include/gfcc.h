@@ -104,7 +104,9 @@ int gfcc_set_stream(gfcc_handle h, void* cuda_stream);
  *   "gmres_fixed"  if > 0: run exactly this many Arnoldi steps in ONE cycle, no stop test, no compaction (timing mode);
  *                  takes effect on every call (a later smaller value is honoured without reallocation)
  *   "x0"           0: zero initial guess, 1: zeroth-order guess b/(omega - i eta + d) (default 1)
- *   "panel_bytes"  upper bound for the (ov x ov) integral panel scratch (default 3.2e9: 5 occupied indices per panel at config 4)
+ *   "panel_bytes"  upper bound for one (ov x ov) integral panel scratch.  Default (option never set): 12.8e9 for the sigma workspace of
+ *                  the DMMA engine (20 occupied indices per panel at config 4) and 3.2e9 for the create-time scratch, the EA panels and
+ *                  the INT8 engine; a value set here applies to all of them
  *   "max_batch"    largest number of right-hand sides processed at once by gfcc_solve_ip (default 256)
  *   "compact"      converged-RHS compaction (iteration counts differ between (omega,p) tasks): when at least
  *                  max(1, compact * active columns) right-hand sides of the batch have met the stop test they are finalised and

@@ -52,7 +52,7 @@ static int ea_ensure_ws(gfcc_ctx* h, EaState& e, int nrhs) {
   if (e.ws_nrhs >= nrhs) return GFCC_OK;
   if (e.ws_nrhs) { cudaStreamSynchronize(h->stream); ea_free_ws(h, e); }
   const long long o = h->o, v = h->v, Q = h->Q, Nc = 2LL * nrhs, ldE = v * Nc, ldO = o * Nc, ov = o * v, vv = v * v;
-  const double budget = h->opt_panel_bytes;
+  const double budget = panel_budget(h, false);
   e.ni = (int)std::max<double>(1, std::min<double>((double)o, std::floor(budget / (8.0 * v * ov))));
   e.na = (int)std::max<double>(1, std::min<double>((double)v, std::floor(budget / (8.0 * v * vv))));
   e.nm = (int)std::max<long long>(1, std::min<long long>(o, (long long)e.na * v / o));   // the (m',n) x (c,d) panel of U lives in PP
@@ -105,7 +105,7 @@ static int ea_prepare(gfcc_ctx* h, EaState& e) {
     TRY(gemm(h, d));
   }
   k_ea_addto<<<nblk(Q * ov), 256, 0, st>>>(Lvo, h->Lm, Q * ov); KLAUNCH(h);
-  const double budget = h->opt_panel_bytes;
+  const double budget = panel_budget(h, false);
   // ---- T_a: X1[(a',e)][(j,b)] = sum_Q Lvv[Q][a][e] L~vo[Q][j][b], antisymmetrised in (a,b) by the scatter; panels over a
   {
     int na = (int)std::max<double>(1, std::min<double>(v, std::floor(budget / (8.0 * v * ov))));

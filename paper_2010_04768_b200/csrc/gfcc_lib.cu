@@ -80,7 +80,7 @@ struct gfcc_ctx {
   int oz_ws_nrhs = 0, oz_ws_ni = 0;
   double st_oz_gemms = 0;
   // ---- options / stats ----
-  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 3.2e9, opt_max_batch = 256, opt_overlap = 0;
+  double opt_m = 50, opt_maxit = 1000, opt_fixed = 0, opt_x0 = 1, opt_panel_bytes = 0 /* 0 = automatic, see panel_budget() */, opt_max_batch = 256, opt_overlap = 0;
   double opt_compact = 0.125, opt_poll = 0, opt_graph = -1, opt_dense = -1;
   // ---- dense Hbar_IP (n x n, row-major) for tiny systems: sigma inside the solver = one GEMM + a shift kernel ----
   double* Hd = nullptr; bool hd_ready = false;
@@ -232,6 +232,12 @@ static void free_workspace(gfcc_ctx* h) {
   h->ws_nrhs = 0;
 }
 
+// byte budget of one panel scratch: the "panel_bytes" option when set, else 12.8 GB for the sigma workspace of the DMMA engine
+// (20 occupied indices per panel at config 4: 33.9 TFLOP/s per step against 33.5 with 5 -- the K2 panel build then fills its
+// 96-row tiles) and 3.2 GB for everything else (create-time scratch, EA panels, INT8 engine)
+static double panel_budget(const gfcc_ctx* h, bool sigma_dmma) {
+  return h->opt_panel_bytes > 0 ? h->opt_panel_bytes : (sigma_dmma ? 12.8e9 : 3.2e9);
+}
 // choose how many occupied indices one (ov x ov) panel covers: as many as the byte budget allows, preferring
 // counts whose consuming GEMM fills whole waves of 148 CTAs.
 static int choose_panel(int o, int v, long long ncols, double budget_bytes) {
@@ -259,8 +265,8 @@ static int ensure_workspace(gfcc_ctx* h, int nrhs, bool need_abi_vecs) {
   if (h->ws_nrhs < nrhs) {
     if (h->ws_nrhs) { cudaStreamSynchronize(h->stream); free_workspace(h); }
     const long long Nc = 2LL * nrhs, big = (long long)o * v * o * Nc;
-    h->panel_ni = h->opt_engine == 1 ? oz_choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes)
-                                     : choose_panel(o, v, (long long)o * Nc, h->opt_panel_bytes);
+    h->panel_ni = h->opt_engine == 1 ? oz_choose_panel(o, v, (long long)o * Nc, panel_budget(h, false))
+                                     : choose_panel(o, v, (long long)o * Nc, panel_budget(h, true));
     h->ws_nrhs = nrhs;   // free_workspace() sizes its bookkeeping with it; reset to 0 there if anything below fails
     int rc = GFCC_OK;
     do {
@@ -738,7 +744,7 @@ static int create_impl(gfcc_ctx* h, const double* fock, const double* T1, const 
   dev_free(h, Mq, Q * ov);
 
   // ---- create-time panel scratch ----
-  const double budget = h->opt_panel_bytes;
+  const double budget = panel_budget(h, false);
   // ---- P5: W_mnij packed ----
   CUDA_TRY(h, cudaMemsetAsync(h->Wp, 0, (size_t)(npair * npair) * 8, st));
   {
